@@ -1,0 +1,176 @@
+/*
+ * rna4r.h -- C ABI of the B200-native two-vector Four-Russians RNA fold.
+ *
+ * Source of every operation: Venkatachalam, Gusfield, Frid, "Faster Algorithms for RNA-folding
+ * using the Four-Russians method" (arxiv 1307.7820), cited below as PAPER.md:<line>.
+ *
+ * Problem (section 2): input a sequence S[1..n] over {A,C,G,U}; output D(1,n),
+ * the largest number of non-crossing complementary (A-U, C-G) base pairs, where
+ *     D(i,i-1) = D(i,i) = 0,
+ *     D(i,j)   = max{ b(S_i,S_j) + D(i+1,j-1),  max_{i+1<=k<=j} D(i,k-1) + D(k,j) }      (eq. (1))
+ * and, on request, the whole upper-triangular table D.
+ *
+ * Method (PAPER.md:62-123 section 3.1, :221-269 section 4): by Lemma 1 adjacent
+ * cells of a row / column differ by 0 or 1, so q consecutive cells are an anchor plus a q-bit
+ * difference vector (v_0 = 0 by definition); eq. (3) replaces q
+ * steps of the inner max by  D(i,l) + D(l+1,j) + R[v][vbar]  with R tabulated once for all
+ * 2^q x 2^q vector pairs.  The fill runs as an anti-diagonal wavefront
+ * (PAPER.md:223-245).
+ *
+ * General rules of this ABI
+ *   - Every pointer argument says "host" or "device".  Device pointers are plain CUDA device
+ *     addresses on the context's device; the caller allocates and owns ALL device buffers
+ *     (sequence, outputs, workspace) and the stream.  The library allocates only what
+ *     rna4r_prepare creates (the R tables) and frees it in rna4r_destroy.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - rna4r_fold / rna4r_fold_batch only ENQUEUE work on `stream` and return; they never
+ *     allocate and never synchronise.  The *_host variants copy in/out and synchronise `stream`.
+ *   - Every function returns 0 (RNA4R_OK) or a negative RNA4R_ERR_* code; nothing throws.
+ *   - There is NO CPU fallback: on a machine without an sm_100 device rna4r_prepare fails with
+ *     RNA4R_ERR_DEVICE and nothing else can be called.
+ *   - Results are deterministic integers (max is order independent): same input, same bits.
+ *   - Input alphabet: bytes A C G U, lower case accepted, T == U.  Any other byte makes that
+ *     sequence's score -1 (and, for rna4r_fold, leaves table_out unspecified); other sequences
+ *     of a batch are unaffected.  n = 0 and n = 1 are valid and score 0.
+ */
+#ifndef RNA4R_H
+#define RNA4R_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes ---- */
+#define RNA4R_OK              0
+#define RNA4R_ERR_BAD_Q      -1   /* q outside 2..12                                           */
+#define RNA4R_ERR_NULL       -2   /* a required pointer is NULL                                */
+#define RNA4R_ERR_BAD_N      -3   /* n < 0, count < 0, or n too large for the chosen engine/q  */
+#define RNA4R_ERR_WORKSPACE  -4   /* workspace_bytes smaller than rna4r_workspace_bytes(...)   */
+#define RNA4R_ERR_CONTEXT    -5   /* NULL / destroyed context                                  */
+#define RNA4R_ERR_CUDA       -6   /* a CUDA runtime call failed (see rna4r_last_cuda_error)    */
+#define RNA4R_ERR_DEVICE     -7   /* no CUDA device, or the device is not compute capability 10.x */
+#define RNA4R_ERR_DTYPE      -8   /* table_dtype not one of RNA4R_TABLE_*                      */
+#define RNA4R_ERR_ENGINE     -9   /* engine id unknown, or the engine does not support this q  */
+
+/* ---- table_out element types ---- */
+#define RNA4R_TABLE_NONE   0
+#define RNA4R_TABLE_INT16  1      /* exact for n <= 65534 (D <= n/2)  */
+#define RNA4R_TABLE_INT32  2
+
+/* ---- fill engines ---- */
+#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 10, else DIAG                         */
+#define RNA4R_ENGINE_TILED  1     /* persistent super-tile wavefront, R resident in shared memory
+                                     (the B200 design)                     */
+#define RNA4R_ENGINE_DIAG   2     /* paper-literal section 4 algorithm: one launch per anti-
+                                     diagonal, one thread per cell, per-cell sliding vectors
+                                     (PAPER.md:249-267); any q in 2..12; the comparison point   */
+
+typedef struct rna4r_ctx rna4r_ctx;   /* opaque; owns the device R tables for one q on one device */
+
+/*
+ * rna4r_prepare -- preprocessing step ("we will run the above algorithm for all
+ * possible vector pairs of length q and store the results in table R"; the
+ * 2^q x 2^q entries are independent).  Builds on `device`, enqueued on `stream`:
+ *   - R : uint8[2^q][2^q], R[v][vbar] = max-val of the listing PAPER.md:94-111, index bit k = |v_k|;
+ *   - the compact reachable quadrant the fill kernels stage in shared memory
+ *     (v_0 = vbar_0 = 0): Rc[h][w] = R[2h][2w], 2^(q-1) x 2^(q-1) entries.
+ * q: host int, 2..12.  device: CUDA ordinal.  out: host pointer receiving the context.
+ * Errors: BAD_Q, NULL, DEVICE, CUDA.
+ */
+int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out);
+
+/* Frees the context and its device tables (synchronises the device).  Errors: CONTEXT. */
+int rna4r_destroy(rna4r_ctx *ctx);
+
+/* q of the context (or RNA4R_ERR_CONTEXT). */
+int rna4r_q(const rna4r_ctx *ctx);
+
+/* Device pointer to R (uint8[2^q][2^q], row = horizontal vector v, column = vertical vector vbar),
+ * or NULL.  Valid until rna4r_destroy; ordered after rna4r_prepare's stream work. */
+const uint8_t *rna4r_table(const rna4r_ctx *ctx);
+
+/* Device pointer to the compact table Rc (uint8[2^(q-1)][2^(q-1)]), or NULL. */
+const uint8_t *rna4r_table_compact(const rna4r_ctx *ctx);
+
+/* Copies R (compact = 0: 2^q * 2^q bytes) or Rc (compact = 1: 2^(q-1) * 2^(q-1) bytes) into HOST memory
+ * dst_host after synchronising the device (a test / inspection helper).  Errors: CONTEXT, NULL, CUDA. */
+int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact);
+
+/* Selects the fill engine (RNA4R_ENGINE_*) for later fold calls.  Errors: CONTEXT, ENGINE. */
+int rna4r_set_engine(rna4r_ctx *ctx, int engine);
+int rna4r_engine(const rna4r_ctx *ctx);   /* the engine fold calls will use (resolved, never AUTO) */
+
+/*
+ * Workspace size in bytes for `count` sequences each of length <= n_max with the context's current
+ * engine (an upper bound; 0 on error).  rna4r_workspace_bytes_batch gives the exact size for given
+ * lengths (lens_host: host int32[count]).  The workspace needs 256-byte alignment and holds only
+ * scratch: its contents are undefined before and after a call.
+ */
+size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count);
+size_t rna4r_workspace_bytes_batch(const rna4r_ctx *ctx, const int32_t *lens_host, int count);
+
+/*
+ * rna4r_fold -- one fold (problem statement PAPER.md:45-54; wavefront PAPER.md:223-269).
+ *   seq_dev       device uint8[n]: the bases S_1..S_n as ASCII bytes (read only).
+ *   n             host int, 0 <= n <= 65534.
+ *   score_out_dev device int32[1]: receives D(1,n) (-1 if seq holds an invalid byte).
+ *   table_out_dev device or NULL: n*n elements row-major, entry [i-1][j-1] = D(i,j) for i <= j,
+ *                 0 below the diagonal; element type given by table_dtype (RNA4R_TABLE_*;
+ *                 pass RNA4R_TABLE_NONE with NULL).
+ *   workspace_dev device scratch of >= rna4r_workspace_bytes(ctx, n, 1) bytes.
+ * Errors: CONTEXT, NULL, BAD_N, DTYPE, WORKSPACE, CUDA (launch failure).
+ */
+int rna4r_fold(rna4r_ctx *ctx, const uint8_t *seq_dev, int n,
+               int32_t *score_out_dev, void *table_out_dev, int table_dtype,
+               void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/*
+ * rna4r_fold_batch -- `count` independent folds in one call (BASELINE.json north_star; each fold
+ * is PAPER.md:45-54).  Sequence t is seqs_dev[offsets_dev[t] .. offsets_dev[t+1]).
+ *   seqs_dev       device uint8[offsets[count]]: concatenated bases.
+ *   offsets_dev    device int64[count+1]: start offsets, offsets[0] = 0, non-decreasing.
+ *   lens_host      HOST int32[count]: lens_host[t] = offsets[t+1]-offsets[t]; host memory so the
+ *                  library can size and validate the work without a device synchronisation.
+ *   scores_out_dev device int32[count]: D(1,n_t) per sequence (-1 for an invalid sequence).
+ *   workspace_dev  device scratch of >= rna4r_workspace_bytes_batch(ctx, lens_host, count).
+ * Errors: CONTEXT, NULL, BAD_N, WORKSPACE, CUDA.
+ */
+int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *offsets_dev,
+                     const int32_t *lens_host, int count, int32_t *scores_out_dev,
+                     void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/*
+ * Host-buffer variants (the end-to-end path): the sequence(s) are copied host->device into the
+ * workspace, folded, the score(s) (and table) copied device->host, and `stream` is synchronised
+ * before returning.  Host buffers should be pinned for full copy bandwidth but need not be.
+ * Workspace: rna4r_workspace_bytes_host(ctx, total_bases, count, table_elems_bytes) extra bytes on
+ * top of the device-side requirement are included by the *_host size queries below.
+ *   table_out_host (rna4r_fold_host only): host n*n elements or NULL.
+ */
+size_t rna4r_workspace_bytes_host(const rna4r_ctx *ctx, const int32_t *lens_host, int count, int table_dtype);
+int rna4r_fold_host(rna4r_ctx *ctx, const uint8_t *seq_host, int n,
+                    int32_t *score_out_host, void *table_out_host, int table_dtype,
+                    void *workspace_dev, size_t workspace_bytes, void *stream);
+int rna4r_fold_batch_host(rna4r_ctx *ctx, const uint8_t *seqs_host, const int32_t *lens_host, int count,
+                          int32_t *scores_out_host,
+                          void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/* Number of kernel launches the most recent fold call enqueued (for accounting), or < 0. */
+int rna4r_last_launch_count(const rna4r_ctx *ctx);
+
+/* cudaError_t of the most recent failing CUDA call on this context (0 if none). */
+int rna4r_last_cuda_error(const rna4r_ctx *ctx);
+
+/* Static string for an error code. */
+const char *rna4r_strerror(int code);
+
+/* Library / build identification, e.g. "rna4r 0.1 sm_100a". */
+const char *rna4r_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RNA4R_H */

@@ -1,0 +1,337 @@
+// api.cu -- the C ABI of librna4r.so (include/rna4r.h): context, workspace planning, dispatch.
+#include "common.cuh"
+#include "rtable.cuh"
+#include "diag_engine.cuh"
+#include "tiled_engine.cuh"
+
+#include <new>
+
+namespace {
+
+constexpr int kDelta = 4;   // product stages every kDelta steps
+
+inline bool ctx_ok(const rna4r_ctx *c) { return c && c->magic == RNA4R_MAGIC; }
+
+template <typename F>
+auto dispatch_q(int q, F &&f) -> decltype(f(std::integral_constant<int, 8>{}))
+{
+    switch (q) {
+    case 2: return f(std::integral_constant<int, 2>{});
+    case 3: return f(std::integral_constant<int, 3>{});
+    case 4: return f(std::integral_constant<int, 4>{});
+    case 5: return f(std::integral_constant<int, 5>{});
+    case 6: return f(std::integral_constant<int, 6>{});
+    case 7: return f(std::integral_constant<int, 7>{});
+    case 8: return f(std::integral_constant<int, 8>{});
+    case 9: return f(std::integral_constant<int, 9>{});
+    default: return f(std::integral_constant<int, 10>{});
+    }
+}
+
+// largest n the tagged 32-bit words of the tiled engine can hold: anchor sums + q < 2^(32-SH)
+inline int tiled_max_n(int q)
+{
+    const int sh = 2 * (q - 1);
+    const long long lim = (1ll << (32 - sh)) - 1 - q;   // max value of A + B + rv
+    long long n = 2 * lim;                              // D <= n/2
+    if (n > 65534) n = 65534;
+    return (int)n;
+}
+
+size_t tiled_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_single)
+{
+    return dispatch_q(ctx->q, [&](auto Q) { return tiled::workspace_bytes_q<decltype(Q)::value>(kDelta, lens, count, n_single); });
+}
+
+size_t engine_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_single)
+{
+    if (ctx->engine == RNA4R_ENGINE_TILED) return tiled_ws(ctx, lens, count, n_single);
+    // DIAG: sequences of a batch are folded one after another, each in its own slice
+    size_t total = 0;
+    for (int t = 0; t < count; ++t) total += diag_ws_layout(nullptr, lens ? lens[t] : n_single).bytes;
+    return total;
+}
+
+int check_n(const rna4r_ctx *ctx, int n)
+{
+    if (n < 0 || n > 65534) return RNA4R_ERR_BAD_N;
+    if (ctx->engine == RNA4R_ENGINE_TILED && n > tiled_max_n(ctx->q)) return RNA4R_ERR_BAD_N;
+    return RNA4R_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *rna4r_version(void) { return "rna4r 0.1 sm_100a"; }
+
+const char *rna4r_strerror(int code)
+{
+    switch (code) {
+    case RNA4R_OK: return "ok";
+    case RNA4R_ERR_BAD_Q: return "q outside 2..12";
+    case RNA4R_ERR_NULL: return "required pointer is NULL";
+    case RNA4R_ERR_BAD_N: return "bad n or count (negative, or too large for this engine and q)";
+    case RNA4R_ERR_WORKSPACE: return "workspace too small";
+    case RNA4R_ERR_CONTEXT: return "invalid context";
+    case RNA4R_ERR_CUDA: return "CUDA runtime error";
+    case RNA4R_ERR_DEVICE: return "no sm_100 CUDA device (there is no CPU fallback)";
+    case RNA4R_ERR_DTYPE: return "bad table dtype";
+    case RNA4R_ERR_ENGINE: return "unknown engine, or engine does not support this q";
+    default: return "unknown error code";
+    }
+}
+
+int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
+{
+    if (!out) return RNA4R_ERR_NULL;
+    *out = nullptr;
+    if (q < 2 || q > 12) return RNA4R_ERR_BAD_Q;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return RNA4R_ERR_DEVICE;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return RNA4R_ERR_DEVICE;
+    if (prop.major != 10) return RNA4R_ERR_DEVICE;   // sm_100a code only; no fallback path exists
+    rna4r_ctx *ctx = new (std::nothrow) rna4r_ctx();
+    if (!ctx) return RNA4R_ERR_CUDA;
+    ctx->magic = RNA4R_MAGIC; ctx->q = q; ctx->device = device;
+    ctx->engine = (q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->R = ctx->Rc = ctx->Rc4 = nullptr;
+    ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t N = (size_t)1 << q, M = (size_t)1 << (q - 1);
+    auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4); delete ctx; return RNA4R_ERR_CUDA; };
+    cudaError_t e;
+    if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&ctx->R, N * N)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&ctx->Rc, M * M < 16 ? 16 : M * M)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&ctx->Rc4, M * M / 2 < 16 ? 16 : M * M / 2)) != cudaSuccess) return fail(e);
+    {
+        const size_t total = N * N;
+        int blocks = (int)((total + 255) / 256); if (blocks > 148 * 16) blocks = 148 * 16;
+        rna4r_build_rtable_kernel<<<blocks, 256, 0, st>>>(q, ctx->R);
+        const size_t tc = M * M;
+        blocks = (int)((tc + 255) / 256); if (blocks > 148 * 16) blocks = 148 * 16;
+        rna4r_build_compact_kernel<<<blocks, 256, 0, st>>>(q, ctx->R, ctx->Rc);
+        rna4r_pack_nibbles_kernel<<<blocks, 256, 0, st>>>(tc, ctx->Rc, ctx->Rc4);
+        if ((e = cudaGetLastError()) != cudaSuccess) return fail(e);
+        ctx->last_launches = 3;
+    }
+    *out = ctx;
+    return RNA4R_OK;
+}
+
+int rna4r_destroy(rna4r_ctx *ctx)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4);
+    ctx->magic = 0;
+    delete ctx;
+    return RNA4R_OK;
+}
+
+int rna4r_q(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->q : RNA4R_ERR_CONTEXT; }
+const uint8_t *rna4r_table(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->R : nullptr; }
+const uint8_t *rna4r_table_compact(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->Rc : nullptr; }
+int rna4r_engine(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->engine : RNA4R_ERR_CONTEXT; }
+int rna4r_last_launch_count(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->last_launches : RNA4R_ERR_CONTEXT; }
+int rna4r_last_cuda_error(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->last_cuda_error : RNA4R_ERR_CONTEXT; }
+
+int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (!dst_host) return RNA4R_ERR_NULL;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    RNA4R_CUDA(ctx, cudaDeviceSynchronize());
+    const size_t side = (size_t)1 << (compact ? ctx->q - 1 : ctx->q);
+    RNA4R_CUDA(ctx, cudaMemcpy(dst_host, compact ? ctx->Rc : ctx->R, side * side, cudaMemcpyDeviceToHost));
+    return RNA4R_OK;
+}
+
+int rna4r_set_engine(rna4r_ctx *ctx, int engine)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (engine == RNA4R_ENGINE_AUTO) engine = (ctx->q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
+    if (engine != RNA4R_ENGINE_TILED && engine != RNA4R_ENGINE_DIAG) return RNA4R_ERR_ENGINE;
+    if (engine == RNA4R_ENGINE_TILED && ctx->q > 10) return RNA4R_ERR_ENGINE;
+    ctx->engine = engine;
+    return RNA4R_OK;
+}
+
+size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count)
+{
+    if (!ctx_ok(ctx) || n_max < 0 || count < 0 || n_max > 65534) return 0;
+    if (count == 0) return 256;
+    if (ctx->engine == RNA4R_ENGINE_TILED) {
+        // every sequence at n_max: per-sequence cost is monotone in n
+        return (size_t)count * (tiled_ws(ctx, nullptr, 1, n_max)) ;
+    }
+    return (size_t)count * diag_ws_layout(nullptr, n_max).bytes;
+}
+
+size_t rna4r_workspace_bytes_batch(const rna4r_ctx *ctx, const int32_t *lens_host, int count)
+{
+    if (!ctx_ok(ctx) || count < 0 || (!lens_host && count > 0)) return 0;
+    if (count == 0) return 256;
+    for (int t = 0; t < count; ++t) if (lens_host[t] < 0 || lens_host[t] > 65534) return 0;
+    return engine_ws(ctx, lens_host, count, 0);
+}
+
+int rna4r_fold(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_out_dev,
+               void *table_out_dev, int table_dtype, void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (!score_out_dev || !workspace_dev || (!seq_dev && n > 0)) return RNA4R_ERR_NULL;
+    int rc = check_n(ctx, n);
+    if (rc != RNA4R_OK) return rc;
+    if (table_dtype != RNA4R_TABLE_NONE && table_dtype != RNA4R_TABLE_INT16 && table_dtype != RNA4R_TABLE_INT32) return RNA4R_ERR_DTYPE;
+    if ((table_dtype == RNA4R_TABLE_NONE) != (table_out_dev == nullptr)) return table_out_dev ? RNA4R_ERR_DTYPE : RNA4R_ERR_NULL;
+    if (workspace_bytes < engine_ws(ctx, nullptr, 1, n)) return RNA4R_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (ctx->engine == RNA4R_ENGINE_DIAG)
+        return diag_fold_enqueue(ctx, seq_dev, n, score_out_dev, table_out_dev, table_dtype, workspace_dev, st);
+    if (table_out_dev && n > 0) {
+        const size_t es = table_dtype == RNA4R_TABLE_INT16 ? 2 : 4;
+        RNA4R_CUDA(ctx, cudaMemsetAsync(table_out_dev, 0, (size_t)n * n * es, st));   // zeros below the diagonal
+    }
+    return dispatch_q(ctx->q, [&](auto Q) {
+        return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seq_dev, nullptr, nullptr, 1, n, score_out_dev,
+                                                    table_out_dev, table_dtype, workspace_dev, st);
+    });
+}
+
+int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *offsets_dev, const int32_t *lens_host,
+                     int count, int32_t *scores_out_dev, void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (count < 0) return RNA4R_ERR_BAD_N;
+    if (count == 0) { ctx->last_launches = 0; return RNA4R_OK; }
+    if (!offsets_dev || !lens_host || !scores_out_dev || !workspace_dev) return RNA4R_ERR_NULL;
+    size_t total_bases = 0;
+    for (int t = 0; t < count; ++t) {
+        int rc = check_n(ctx, lens_host[t]);
+        if (rc != RNA4R_OK) return rc;
+        total_bases += (size_t)lens_host[t];
+    }
+    if (!seqs_dev && total_bases > 0) return RNA4R_ERR_NULL;
+    if (workspace_bytes < engine_ws(ctx, lens_host, count, 0)) return RNA4R_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (ctx->engine == RNA4R_ENGINE_DIAG) {
+        size_t off = 0, ws_off = 0;
+        int launches = 0;
+        for (int t = 0; t < count; ++t) {
+            int rc = diag_fold_enqueue(ctx, seqs_dev + off, lens_host[t], scores_out_dev + t, nullptr, RNA4R_TABLE_NONE,
+                                       (char *)workspace_dev + ws_off, st);
+            if (rc != RNA4R_OK) return rc;
+            launches += ctx->last_launches;
+            off += (size_t)lens_host[t];
+            ws_off += diag_ws_layout(nullptr, lens_host[t]).bytes;
+        }
+        ctx->last_launches = launches;
+        return RNA4R_OK;
+    }
+    return dispatch_q(ctx->q, [&](auto Q) {
+        return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
+                                                    nullptr, RNA4R_TABLE_NONE, workspace_dev, st);
+    });
+}
+
+// ---- host-buffer variants: staging area at the END of the workspace --------------------------------
+static size_t host_staging_bytes(size_t total_bases, int count, size_t table_bytes)
+{
+    return align_up(total_bases + 16, 256) + align_up((size_t)(count + 1) * 8, 256) + align_up((size_t)count * 4 + 16, 256) + align_up(table_bytes, 256);
+}
+
+size_t rna4r_workspace_bytes_host(const rna4r_ctx *ctx, const int32_t *lens_host, int count, int table_dtype)
+{
+    if (!ctx_ok(ctx) || count < 0 || (!lens_host && count > 0)) return 0;
+    size_t total_bases = 0;
+    for (int t = 0; t < count; ++t) { if (lens_host[t] < 0 || lens_host[t] > 65534) return 0; total_bases += (size_t)lens_host[t]; }
+    size_t table_bytes = 0;
+    if (table_dtype != RNA4R_TABLE_NONE && count == 1)
+        table_bytes = (size_t)lens_host[0] * lens_host[0] * (table_dtype == RNA4R_TABLE_INT16 ? 2 : 4);
+    const size_t core = count ? engine_ws(ctx, lens_host, count, 0) : 256;
+    return align_up(core, 256) + host_staging_bytes(total_bases, count, table_bytes);
+}
+
+int rna4r_fold_host(rna4r_ctx *ctx, const uint8_t *seq_host, int n, int32_t *score_out_host,
+                    void *table_out_host, int table_dtype, void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (!score_out_host || !workspace_dev || (!seq_host && n > 0)) return RNA4R_ERR_NULL;
+    int rc = check_n(ctx, n);
+    if (rc != RNA4R_OK) return rc;
+    if (table_dtype != RNA4R_TABLE_NONE && table_dtype != RNA4R_TABLE_INT16 && table_dtype != RNA4R_TABLE_INT32) return RNA4R_ERR_DTYPE;
+    if ((table_dtype == RNA4R_TABLE_NONE) != (table_out_host == nullptr)) return table_out_host ? RNA4R_ERR_DTYPE : RNA4R_ERR_NULL;
+    const int32_t len1 = n;
+    if (workspace_bytes < rna4r_workspace_bytes_host(ctx, &len1, 1, table_dtype)) return RNA4R_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t core = align_up(engine_ws(ctx, nullptr, 1, n), 256);
+    char *stg = (char *)workspace_dev + core;
+    uint8_t *seq_dev = (uint8_t *)stg; stg += align_up((size_t)n + 16, 256);
+    stg += align_up(2 * 8, 256);
+    int32_t *score_dev = (int32_t *)stg; stg += align_up(4 + 16, 256);
+    void *table_dev = table_out_host ? (void *)stg : nullptr;
+    const size_t table_bytes = table_out_host ? (size_t)n * n * (table_dtype == RNA4R_TABLE_INT16 ? 2 : 4) : 0;
+    if (n > 0) RNA4R_CUDA(ctx, cudaMemcpyAsync(seq_dev, seq_host, (size_t)n, cudaMemcpyHostToDevice, st));
+    rc = rna4r_fold(ctx, seq_dev, n, score_dev, table_dev, table_dtype, workspace_dev, core, st);
+    if (rc != RNA4R_OK) return rc;
+    const int launches = ctx->last_launches;
+    RNA4R_CUDA(ctx, cudaMemcpyAsync(score_out_host, score_dev, 4, cudaMemcpyDeviceToHost, st));
+    if (table_bytes) RNA4R_CUDA(ctx, cudaMemcpyAsync(table_out_host, table_dev, table_bytes, cudaMemcpyDeviceToHost, st));
+    RNA4R_CUDA(ctx, cudaStreamSynchronize(st));
+    ctx->last_launches = launches;
+    return RNA4R_OK;
+}
+
+int rna4r_fold_batch_host(rna4r_ctx *ctx, const uint8_t *seqs_host, const int32_t *lens_host, int count,
+                          int32_t *scores_out_host, void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (count < 0) return RNA4R_ERR_BAD_N;
+    if (count == 0) return RNA4R_OK;
+    if (!lens_host || !scores_out_host || !workspace_dev) return RNA4R_ERR_NULL;
+    size_t total_bases = 0;
+    for (int t = 0; t < count; ++t) {
+        int rc = check_n(ctx, lens_host[t]);
+        if (rc != RNA4R_OK) return rc;
+        total_bases += (size_t)lens_host[t];
+    }
+    if (!seqs_host && total_bases > 0) return RNA4R_ERR_NULL;
+    if (workspace_bytes < rna4r_workspace_bytes_host(ctx, lens_host, count, RNA4R_TABLE_NONE)) return RNA4R_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t core = align_up(engine_ws(ctx, lens_host, count, 0), 256);
+    char *stg = (char *)workspace_dev + core;
+    uint8_t *seqs_dev = (uint8_t *)stg; stg += align_up(total_bases + 16, 256);
+    int64_t *offs_dev = (int64_t *)stg; stg += align_up((size_t)(count + 1) * 8, 256);
+    int32_t *scores_dev = (int32_t *)stg;
+    // offsets are derived from lens on the host (count+1 int64) and copied with the bases
+    int64_t *offs_host = new (std::nothrow) int64_t[(size_t)count + 1];
+    if (!offs_host) return RNA4R_ERR_CUDA;
+    offs_host[0] = 0;
+    for (int t = 0; t < count; ++t) offs_host[t + 1] = offs_host[t] + lens_host[t];
+    cudaError_t e = cudaMemcpyAsync(offs_dev, offs_host, (size_t)(count + 1) * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && total_bases) e = cudaMemcpyAsync(seqs_dev, seqs_host, total_bases, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // offs_host is pageable: make sure the copy has consumed it
+    delete[] offs_host;
+    if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return RNA4R_ERR_CUDA; }
+    int rc = rna4r_fold_batch(ctx, seqs_dev, offs_dev, lens_host, count, scores_dev, workspace_dev, core, st);
+    if (rc != RNA4R_OK) return rc;
+    const int launches = ctx->last_launches;
+    RNA4R_CUDA(ctx, cudaMemcpyAsync(scores_out_host, scores_dev, (size_t)count * 4, cudaMemcpyDeviceToHost, st));
+    RNA4R_CUDA(ctx, cudaStreamSynchronize(st));
+    ctx->last_launches = launches;
+    return RNA4R_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,57 @@
+// common.cuh -- context, error handling and small device helpers shared by the rna4r kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/rna4r.h"
+
+struct rna4r_ctx {
+    uint32_t magic;
+    int q;
+    int device;
+    int engine;              // resolved engine (never AUTO)
+    int sm_count;
+    uint8_t *R;              // device uint8[2^q][2^q]
+    uint8_t *Rc;             // device uint8[2^(q-1)][2^(q-1)]   reachable quadrant, Rc[h][w] = R[2h][2w]
+    uint8_t *Rc4;            // device nibble-packed Rc (two entries per byte), only when 2(q-1) > 16
+    int last_launches;
+    int last_cuda_error;
+    int tiled_blocks_per_sm; // occupancy of the tiled fill kernel for this q (0 = not queried yet)
+};
+static const uint32_t RNA4R_MAGIC = 0x52344e41u;
+
+#define RNA4R_CUDA(ctx, call)                                             \
+    do {                                                                  \
+        cudaError_t e__ = (call);                                         \
+        if (e__ != cudaSuccess) {                                         \
+            if (ctx) (ctx)->last_cuda_error = (int)e__;                   \
+            return RNA4R_ERR_CUDA;                                        \
+        }                                                                 \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// base byte -> code 0..3 (A,C,G,U/T, either case); 4 = not a base (reading g4)
+__device__ __forceinline__ int rna4r_base_code(uint8_t c)
+{
+    switch (c) {
+    case 'A': case 'a': return 0;
+    case 'C': case 'c': return 1;
+    case 'G': case 'g': return 2;
+    case 'U': case 'u': case 'T': case 't': return 3;
+    default: return 4;
+    }
+}
+// b(x,y) of eq. (1): A-U and C-G pair; code 4 (padding / invalid) pairs with nothing
+__device__ __forceinline__ int rna4r_pair(int x, int y) { return (x + y == 3) ? 1 : 0; }
+
+__device__ __forceinline__ int ld_acquire_gpu(const int *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu(int *p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}

@@ -1,0 +1,775 @@
+// tiled_engine.cuh -- RNA4R_ENGINE_TILED: the B200 design of the two-vector Four-Russians fill.
+//
+// Coordinates.  The paper's D(i,j) (1-based) is held as a matrix M(r,c) = D(r+1, c),
+// r,c in [0,n]: M(r,c) = 0 for c <= r+1, and eq. (1) becomes a pure max-plus closure
+//     M(r,c) = max{ b(S[r],S[c-1]) + M(r+1,c-1),  max_{r<t<c} M(r,t) + M(t,c) }.
+// With this shift the paper's two offset groupings (columns (0..q-1),(q..2q-1),.. and rows
+// (1..q),(q+1..2q),..) are the SAME grouping of the split index t: group g is
+// t in [gq, gq+q).
+//
+// Two-vector step (eq. (3)).  For group g, row r, column c:
+//     max_{t in g} M(r,t)+M(t,c) = M(r,gq) + M(gq,c) + Rc[h][v]
+//   h = the q-1 horizontal difference bits of M(r,gq..gq+q-1)  (v_1..v_{q-1};  v_0 = 0)
+//   v = the q-1 vertical   difference bits of M(gq..gq+q-1,c)  (|vbar_1|..|vbar_{q-1}|; vbar_0 = 0)
+// Each (row, group) is one 32-bit word  W = M(r,gq) << SH | h << HB  and each (group, column) one
+// word X = M(gq,c) << SH | v  (HB = q-1, SH = 2*HB).  Then S = W + X carries the table index in its
+// low SH bits and the anchor sum above them, and  S + (Rc[idx] << SH)  is the candidate, still
+// tagged with harmless low bits: one add, one mask, one byte gather, one shift-add, one max.
+//
+// Decomposition.  Super-tiles of T = 8q cells (8 groups) per side.  For super-tile (I,J), I < J:
+//   * every group lying in a block K strictly between I and J is a "full group" for ALL T*T cells
+//     (Alg. 1 lines 15-19): a max-plus product of the row panel of (I,K) with the
+//     column panel of (K,J) through Rc -- the bulk, no dependency inside the tile;
+//   * groups inside blocks I and J depend on cells of (I,J) itself: the closure, a 2T-1 step
+//     anti-diagonal wavefront inside the CTA.  The paper's residual loops
+//      are done as MASKED lookups: a partial group is a lookup whose not
+//     yet known difference bits are zero (DESIGN.md section 4.3 proves this is exact).
+// Work units (tasks) are listed step by step (step = super-tile diagonal J-I), claimed in order from
+// one atomic counter by a persistent grid, and ordered by acquire/release flags instead of a grid
+// barrier per diagonal ("Synchronize with other processes").
+#pragma once
+#include "common.cuh"
+
+namespace tiled {
+
+template <int Q>
+struct Cfg {
+    static constexpr int T = 8 * Q;            // cells per super-tile side
+    static constexpr int HB = Q - 1;           // informative bits per vector
+    static constexpr int SH = 2 * HB;          // table index bits
+    static constexpr uint32_t IDXMASK = (1u << SH) - 1u;
+    static constexpr bool NIBBLE = (SH > 16);  // q = 10: nibble-packed table (128 KB)
+    static constexpr int TBL_BYTES = NIBBLE ? (1 << SH) / 2 : (1 << SH);
+    static constexpr int NTHR = 4 * T;         // threads per CTA
+    static constexpr int RPT = 2 * Q;          // rows per thread in the product phase
+    static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
+    static constexpr int VP = T + 2;           // pitch of the value array (int16)
+    static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
+    static constexpr int REC_BYTES = 2 * PANEL_WORDS * 4 + 2 * T * 2;   // PH, PV, top row, right column
+    static constexpr size_t SMEM_BYTES =
+        (size_t)((TBL_BYTES + 15) / 16 * 16) + 2 * 16 * TP * 4 + 2 * T * 4 + (size_t)(T + 1) * VP * 2 + 2 * 2 * PANEL_WORDS * 4 + 2 * T + 64;
+};
+
+struct SeqInfo {
+    int n;         // sequence length
+    int nt;        // super-tiles per side = n / T + 1
+    int sbase;     // index of this sequence's first super-tile record
+    int cbase;     // offset of this sequence's codes
+    int invalid;   // != 0 if a byte was not a base
+    int pad[3];
+};
+
+// header of the plan area (zeroed by one memset at the start of every fold)
+struct PlanHdr {
+    int counter;    // task claim counter
+    int total;      // number of tasks
+    int ntiles;     // allocation cursor: super-tile records
+    int ncodes;     // allocation cursor: code bytes
+    int pad[4];
+};
+
+constexpr int TASK_CLOSE = 0;
+constexpr int TASK_PROD = 1;
+
+struct Params {
+    const uint8_t *seqs;
+    const int64_t *offsets;   // device [count+1], or NULL for a single sequence of length n_single
+    int n_single;
+    int count;
+    int max_nt;
+    int delta;
+    PlanHdr *hdr;
+    int *stepC;       // [max_nt] closure tasks per step, then segment base
+    int *stepP;       // [max_nt] product tasks per step, then segment base
+    int *curC;        // [max_nt] fill cursors
+    int *curP;
+    SeqInfo *seqinfo; // [count]
+    int *done;        // [tiles] 1 when the super-tile's panels are published
+    int *accstage;    // [tiles] product stages merged into acc so far
+    int4 *tasks;      // {seq, I | J << 16, kind, stage}
+    int8_t *codes;    // per sequence nt*T codes (4 = padding)
+    uint8_t *recs;    // super-tile records
+    int16_t *acc;     // [tiles][T*T] bulk partial maxima
+    const uint8_t *tbl;   // compact table in global memory (byte or nibble form)
+    int32_t *scores;
+    void *table_out;
+    int table_dtype;
+};
+
+__host__ __device__ inline int nstages(int dp, int delta)
+{
+    // product stages of a target on super-tile diagonal dp: stage s runs at step
+    // dp-1-s*delta and covers member diagonals m in [max(hi-delta+1, ceil(dp/2)), hi], hi = dp-2-s*delta
+    const int mmin = (dp + 1) / 2;
+    if (dp - 2 < mmin) return 0;
+    return (dp - 2 - mmin) / delta + 1;
+}
+__host__ __device__ inline int tri_index(int nt, int I, int J) { return I * nt - (I * (I - 1)) / 2 + (J - I); }
+
+// ------------------------------------------------------------------------------------------------
+// planning kernels (tiny): per-sequence geometry, per-step task counts, task list
+// ------------------------------------------------------------------------------------------------
+template <int Q>
+__global__ void plan_seq_kernel(Params p)
+{
+    constexpr int T = Cfg<Q>::T;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= p.count) return;
+    const int n = p.offsets ? (int)(p.offsets[t + 1] - p.offsets[t]) : p.n_single;
+    const int nt = n / T + 1;
+    SeqInfo si;
+    si.n = n; si.nt = nt; si.invalid = 0; si.pad[0] = si.pad[1] = si.pad[2] = 0;
+    si.sbase = atomicAdd(&p.hdr->ntiles, nt * (nt + 1) / 2);
+    si.cbase = atomicAdd(&p.hdr->ncodes, nt * T);
+    p.seqinfo[t] = si;
+    for (int D = 0; D < nt; ++D) {
+        atomicAdd(&p.stepC[D], nt - D);
+        int np = 0;
+        for (int s = 0;; ++s) {
+            const int dp = D + 1 + s * p.delta;
+            if (dp > nt - 1) break;
+            if (s < nstages(dp, p.delta)) np += nt - dp;
+        }
+        if (np) atomicAdd(&p.stepP[D], np);
+    }
+}
+
+__global__ void plan_scan_kernel(Params p)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int base = 0;
+    for (int D = 0; D < p.max_nt; ++D) {
+        const int c = p.stepC[D], q = p.stepP[D];
+        p.stepC[D] = base; p.curC[D] = base; base += c;
+        p.stepP[D] = base; p.curP[D] = base; base += q;
+    }
+    p.hdr->total = base;
+}
+
+template <int Q>
+__global__ void plan_fill_kernel(Params p)
+{
+    // block <-> (sequence t, step D)
+    const int t = blockIdx.x / p.max_nt, D = blockIdx.x % p.max_nt;
+    const SeqInfo si = p.seqinfo[t];
+    const int nt = si.nt;
+    if (D >= nt) return;
+    __shared__ int s_slot;
+    if (threadIdx.x == 0) s_slot = atomicAdd(&p.curC[D], nt - D);
+    __syncthreads();
+    for (int I = threadIdx.x; I < nt - D; I += blockDim.x)
+        p.tasks[s_slot + I] = make_int4(t, I | ((I + D) << 16), TASK_CLOSE, 0);
+    for (int s = 0;; ++s) {
+        const int dp = D + 1 + s * p.delta;
+        if (dp > nt - 1) break;
+        if (s >= nstages(dp, p.delta)) continue;
+        __syncthreads();
+        if (threadIdx.x == 0) s_slot = atomicAdd(&p.curP[D], nt - dp);
+        __syncthreads();
+        for (int I = threadIdx.x; I < nt - dp; I += blockDim.x)
+            p.tasks[s_slot + I] = make_int4(t, I | ((I + dp) << 16), TASK_PROD, s);
+    }
+}
+
+// bases -> codes, padded with 4 up to nt*T; flags invalid bytes (reading g4)
+template <int Q>
+__global__ void encode_kernel(Params p)
+{
+    constexpr int T = Cfg<Q>::T;
+    const int t = blockIdx.y;
+    const SeqInfo si = p.seqinfo[t];
+    const int len = si.nt * T;
+    const uint8_t *src = p.seqs + (p.offsets ? p.offsets[t] : 0);
+    bool bad = false;
+    for (int x = blockIdx.x * blockDim.x + threadIdx.x; x < len; x += gridDim.x * blockDim.x) {
+        int c = 4;
+        if (x < si.n) { c = rna4r_base_code(src[x]); bad |= (c == 4); }
+        p.codes[si.cbase + x] = (int8_t)c;
+    }
+    if (bad) atomicOr(&p.seqinfo[t].invalid, 1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// fill kernel
+// ------------------------------------------------------------------------------------------------
+template <int Q>
+struct Smem {
+    using C = Cfg<Q>;
+    uint8_t *tbl;        // compact table Rc
+    uint32_t *Wst;       // [16][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own)
+    uint32_t *Xst;       // [16][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static)
+    uint32_t *Wp;        // [T] running (partial) row word of the group being filled
+    uint32_t *Xp;        // [T] running (partial) column word
+    int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
+    uint32_t *stg;       // [2][2][PANEL_WORDS] product operands, double buffered: [buf][0]=PH, [buf][1]=PV
+    int8_t *codeR;       // [T] codes of the rows
+    int8_t *codeC;       // [T] codes of the columns
+    int *misc;           // [16]
+    __device__ explicit Smem(uint8_t *base)
+    {
+        uint8_t *p = base;
+        tbl = p; p += (C::TBL_BYTES + 15) / 16 * 16;
+        Wst = (uint32_t *)p; p += 16 * C::TP * 4;
+        Xst = (uint32_t *)p; p += 16 * C::TP * 4;
+        Wp = (uint32_t *)p; p += C::T * 4;
+        Xp = (uint32_t *)p; p += C::T * 4;
+        stg = (uint32_t *)p; p += 2 * 2 * C::PANEL_WORDS * 4;
+        val = (int16_t *)p; p += (C::T + 1) * C::VP * 2;
+        codeR = (int8_t *)p; p += C::T;
+        codeC = (int8_t *)p; p += C::T;
+        misc = (int *)p;
+    }
+};
+
+template <int Q>
+__device__ __forceinline__ uint32_t lookup(const uint8_t *tbl, uint32_t idx)
+{
+    if constexpr (Cfg<Q>::NIBBLE) {
+        const uint32_t w = reinterpret_cast<const uint32_t *>(tbl)[idx >> 3];
+        return (w >> ((idx & 7u) * 4u)) & 15u;
+    } else {
+        return tbl[idx];
+    }
+}
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void wait_flag_ge(const int *flag, int v)
+{
+    while (ld_acquire_gpu(flag) < v) __nanosleep(40);
+}
+
+template <int Q>
+__device__ __forceinline__ const uint8_t *rec_ptr(const Params &p, int sidx) { return p.recs + (size_t)sidx * Cfg<Q>::REC_BYTES; }
+
+// issue the async copy of PH(I,K) and PV(K,J) into stage buffer `buf` (one 16-byte chunk per thread)
+template <int Q>
+__device__ __forceinline__ void load_operands_async(const Params &p, const Smem<Q> &sm, int buf, int sidx_ik, int sidx_kj)
+{
+    using C = Cfg<Q>;
+    const int tid = threadIdx.x;
+    constexpr int CH = C::PANEL_WORDS / 4;        // 16-byte chunks per panel = 2T
+    uint32_t *dst = sm.stg + (size_t)buf * 2 * C::PANEL_WORDS;
+    if (tid < CH) {
+        cp_async16(dst + tid * 4, rec_ptr<Q>(p, sidx_ik) + (size_t)tid * 16);                               // PH of (I,K)
+    } else {
+        const int c = tid - CH;
+        cp_async16(dst + C::PANEL_WORDS + c * 4, rec_ptr<Q>(p, sidx_kj) + (size_t)C::PANEL_WORDS * 4 + (size_t)c * 16);   // PV of (K,J)
+    }
+    cp_async_commit();
+}
+
+// bulk step (a4): acc[rr] = max over the 8 groups of block K, for column jj and rows rb*RPT+rr.
+// acc is kept in the tagged form (value << SH | low bits); unsigned max orders by value.
+template <int Q>
+__device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, uint32_t (&acc)[Cfg<Q>::RPT], int jj, int rb)
+{
+    using C = Cfg<Q>;
+    const uint32_t *PH = sm.stg + (size_t)buf * 2 * C::PANEL_WORDS;
+    const uint32_t *PV = PH + C::PANEL_WORDS;
+#pragma unroll 2
+    for (int g = 0; g < 8; ++g) {
+        const uint32_t X = PV[g * C::T + jj];
+        const uint32_t *wrow = PH + g * C::T + rb * C::RPT;
+        uint32_t w[C::RPT];
+        // the row words are warp-uniform: broadcast vector loads (16 B when RPT % 4 == 0, else 8 B)
+        if constexpr (C::RPT % 4 == 0) {
+#pragma unroll
+            for (int r4 = 0; r4 < C::RPT / 4; ++r4) {
+                const uint4 t4 = reinterpret_cast<const uint4 *>(wrow)[r4];
+                w[4 * r4] = t4.x; w[4 * r4 + 1] = t4.y; w[4 * r4 + 2] = t4.z; w[4 * r4 + 3] = t4.w;
+            }
+        } else {
+#pragma unroll
+            for (int r2 = 0; r2 < C::RPT / 2; ++r2) {
+                const uint2 t2 = reinterpret_cast<const uint2 *>(wrow)[r2];
+                w[2 * r2] = t2.x; w[2 * r2 + 1] = t2.y;
+            }
+        }
+#pragma unroll
+        for (int rr = 0; rr < C::RPT; ++rr) {
+            const uint32_t S = w[rr] + X;
+            const uint32_t rv = lookup<Q>(sm.tbl, S & C::IDXMASK);
+            const uint32_t cand = S + (rv << C::SH);
+            acc[rr] = max(acc[rr], cand);
+        }
+    }
+}
+
+// ---- PROD task: merge the products of newly available middle blocks into the target's acc ----
+template <int Q>
+__device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, int I, int J, int s)
+{
+    using C = Cfg<Q>;
+    const int tid = threadIdx.x;
+    const int nt = si.nt;
+    const int dp = J - I;
+    const int S = nstages(dp, p.delta);
+    const int hi = dp - 2 - s * p.delta;
+    const int lo = max(hi - p.delta + 1, (dp + 1) / 2);
+    const int sidx = si.sbase + tri_index(nt, I, J);
+    const int jj = tid % C::T, rb = tid / C::T;
+    uint32_t acc[C::RPT];
+#pragma unroll
+    for (int rr = 0; rr < C::RPT; ++rr) acc[rr] = 0;
+
+    // K sequence: for m = lo..hi: K = I+m, then K = J-m (if different)
+    const int nk_max = 2 * (hi - lo + 1);
+    int issued = 0, computed = 0;
+    auto kth = [&](int e) -> int {           // e-th block of the sequence, or -1 for the duplicate
+        const int m = lo + (e >> 1);
+        const int K = (e & 1) ? (J - m) : (I + m);
+        if ((e & 1) && (J - m == I + m)) return -1;
+        return K;
+    };
+    // software pipeline: operands of element e+1 are in flight while element e is computed
+    int e_next = 0;
+    auto issue_next = [&]() -> bool {
+        while (e_next < nk_max) {
+            const int K = kth(e_next++);
+            if (K < 0) continue;
+            const int s_ik = si.sbase + tri_index(nt, I, K), s_kj = si.sbase + tri_index(nt, K, J);
+            if (tid == 0) { wait_flag_ge(p.done + s_ik, 1); wait_flag_ge(p.done + s_kj, 1); }
+            __syncthreads();
+            load_operands_async<Q>(p, sm, issued & 1, s_ik, s_kj);
+            ++issued;
+            return true;
+        }
+        return false;
+    };
+    issue_next();
+    while (computed < issued) {
+        const bool more = issue_next();
+        if (more) cp_async_wait<1>(); else cp_async_wait<0>();
+        __syncthreads();
+        product_accumulate<Q>(sm, computed & 1, acc, jj, rb);
+        ++computed;
+        __syncthreads();     // the buffer may be refilled by the next issue
+    }
+    // merge with earlier stages (they ran at earlier steps and own acc until their release)
+    int16_t *accg = p.acc + (size_t)sidx * C::T * C::T;
+    if (s != S - 1) {
+        if (tid == 0) wait_flag_ge(p.accstage + sidx, S - 1 - s);
+        __syncthreads();
+#pragma unroll
+        for (int rr = 0; rr < C::RPT; ++rr) {
+            const int prev = __ldcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj);
+            acc[rr] = max(acc[rr], (uint32_t)prev << C::SH);
+        }
+    }
+#pragma unroll
+    for (int rr = 0; rr < C::RPT; ++rr)
+        __stcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj, (int16_t)(acc[rr] >> C::SH));
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) st_release_gpu(p.accstage + sidx, S - s);
+}
+
+// ---- closure of an off-diagonal super-tile: 2T-1 anti-diagonal steps, 4 threads per cell ----
+template <int Q>
+__device__ void closure_offdiag(const Smem<Q> &sm)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T;
+    const int tid = threadIdx.x;
+    const int jj = tid >> 2, part = tid & 3;
+    const int gj = jj / Q, pj = jj % Q;
+    const int x = jj + 1;
+    for (int s = 0; s < 2 * T - 1; ++s) {
+        const int a = T - 1 - (s - jj);
+        const bool active = (a >= 0) && (a < T);
+        uint32_t best = 0;
+        int ga = 0, pa = 0;
+        if (active) {
+            ga = a / Q; pa = a % Q;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int vg = part + 4 * e;
+                uint32_t W, X;
+                bool ok;
+                if (vg < 8) {        // groups of block I: row words of (I,I), column words of this tile (below a)
+                    ok = (vg > ga) || (vg == ga && pa != Q - 1);
+                    W = sm.Wst[vg * C::TP + a];
+                    X = (vg == ga) ? sm.Xp[jj] : sm.Xst[vg * C::TP + jj];
+                } else {             // groups of block J: row words of this tile (left of jj), column words of (J,J)
+                    const int g2 = vg - 8;
+                    ok = (g2 < gj) || (g2 == gj && pj != 0);
+                    X = sm.Xst[vg * C::TP + jj];
+                    W = (g2 == gj) ? sm.Wp[a] : sm.Wst[vg * C::TP + a];
+                }
+                if (ok) {
+                    const uint32_t S = W + X;
+                    const uint32_t rv = lookup<Q>(sm.tbl, S & C::IDXMASK);
+                    best = max(best, (S >> C::SH) + rv);
+                }
+            }
+        }
+        best = max(best, __shfl_xor_sync(0xffffffffu, best, 1));
+        best = max(best, __shfl_xor_sync(0xffffffffu, best, 2));
+        if (active && part == 0) {
+            int16_t *vrow = sm.val + a * C::VP;
+            const int cur = vrow[x];                                                  // bulk maximum
+            const int dg = vrow[C::VP + x - 1] + rna4r_pair(sm.codeR[a], sm.codeC[jj]);   // b + M(r+1,c-1)
+            const int v = max(max(cur, dg), (int)best);
+            vrow[x] = (int16_t)v;
+            const int left = vrow[x - 1], below = vrow[C::VP + x];
+            // step a6: append the horizontal bit to the row word, the vertical bit to the column word
+            const uint32_t wp = (pj == 0) ? ((uint32_t)v << C::SH)
+                                          : (sm.Wp[a] | ((uint32_t)(v - left) << (C::HB + pj - 1)));
+            sm.Wp[a] = wp;
+            if (pj == Q - 1) sm.Wst[(8 + gj) * C::TP + a] = wp;
+            const uint32_t xp = (pa == Q - 1) ? ((uint32_t)v << C::SH)
+                                              : ((sm.Xp[jj] & C::IDXMASK) | ((uint32_t)(v - below) << pa) | ((uint32_t)v << C::SH));
+            sm.Xp[jj] = xp;
+            if (pa == 0) sm.Xst[ga * C::TP + jj] = xp;
+        }
+        __syncthreads();
+    }
+}
+
+// ---- closure of a diagonal super-tile (I == J): cells with c <= r+1 are 0; steps s = jj - a ----
+template <int Q>
+__device__ void closure_diag(const Smem<Q> &sm)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T;
+    const int tid = threadIdx.x;
+    const int jj = tid >> 2, part = tid & 3;
+    const int gj = jj / Q, pj = jj % Q;
+    const int x = jj + 1;
+    for (int s = 0; s < T; ++s) {
+        const int a = jj - s;
+        const bool active = (a >= 0);
+        uint32_t best = 0;
+        int ga = 0, pa = 0;
+        if (active) {
+            ga = a / Q; pa = a % Q;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int g = part + 4 * e;
+                const bool ok = (g >= ga) && (g <= gj) && !(g == ga && pa == Q - 1) && !(g == gj && pj == 0);
+                if (ok) {
+                    const uint32_t W = (g < gj) ? sm.Wst[(8 + g) * C::TP + a] : sm.Wp[a];
+                    const uint32_t X = (g > ga) ? sm.Xst[g * C::TP + jj] : sm.Xp[jj];
+                    const uint32_t S = W + X;
+                    const uint32_t rv = lookup<Q>(sm.tbl, S & C::IDXMASK);
+                    best = max(best, (S >> C::SH) + rv);
+                }
+            }
+        }
+        best = max(best, __shfl_xor_sync(0xffffffffu, best, 1));
+        best = max(best, __shfl_xor_sync(0xffffffffu, best, 2));
+        if (active && part == 0) {
+            int16_t *vrow = sm.val + a * C::VP;
+            int v = 0;
+            if (s >= 2) {
+                const int dg = vrow[C::VP + x - 1] + rna4r_pair(sm.codeR[a], sm.codeC[jj]);
+                v = max(dg, (int)best);
+            }
+            vrow[x] = (int16_t)v;
+            const int left = vrow[x - 1], below = vrow[C::VP + x];
+            const uint32_t wp = (pj == 0) ? ((uint32_t)v << C::SH)
+                                          : (sm.Wp[a] | ((uint32_t)(v - left) << (C::HB + pj - 1)));
+            sm.Wp[a] = wp;
+            if (pj == Q - 1) sm.Wst[(8 + gj) * C::TP + a] = wp;
+            const uint32_t xp = (pa == Q - 1) ? ((uint32_t)v << C::SH)
+                                              : ((sm.Xp[jj] & C::IDXMASK) | ((uint32_t)(v - below) << pa) | ((uint32_t)v << C::SH));
+            sm.Xp[jj] = xp;
+            if (pa == 0) sm.Xst[ga * C::TP + jj] = xp;
+        }
+        __syncthreads();
+    }
+}
+
+// ---- CLOSE task ----
+template <int Q>
+__device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si, int seq, int I, int J)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T;
+    const int tid = threadIdx.x;
+    const int nt = si.nt;
+    const int dp = J - I;
+    const int sidx = si.sbase + tri_index(nt, I, J);
+
+    // codes of the rows r = I*T + a (base S[r]) and of the columns c = J*T + jj (base S[c-1])
+    if (tid < T) {
+        sm.codeR[tid] = p.codes[si.cbase + I * T + tid];
+        const int c = J * T + tid;
+        sm.codeC[tid] = (c >= 1) ? p.codes[si.cbase + c - 1] : (int8_t)4;
+    }
+
+    if (dp == 0) {
+        // diagonal super-tile: everything starts from zero
+        for (int e = tid; e < (T + 1) * C::VP / 2; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.val)[e] = 0;
+        for (int e = tid; e < 16 * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
+        if (tid < T) { sm.Wp[tid] = 0; sm.Xp[tid] = 0; }
+        __syncthreads();
+        closure_diag<Q>(sm);
+    } else {
+        const int s_left = si.sbase + tri_index(nt, I, J - 1);
+        const int s_below = si.sbase + tri_index(nt, I + 1, J);
+        const int s_ii = si.sbase + tri_index(nt, I, I);
+        const int s_jj = si.sbase + tri_index(nt, J, J);
+        const int S = nstages(dp, p.delta);
+        if (tid == 0) {
+            wait_flag_ge(p.done + s_left, 1);
+            wait_flag_ge(p.done + s_below, 1);
+            wait_flag_ge(p.done + s_ii, 1);
+            wait_flag_ge(p.done + s_jj, 1);
+            if (S > 0) wait_flag_ge(p.accstage + sidx, S);
+        }
+        __syncthreads();
+        // static words: row words of (I,I) -> Wst[0..7], column words of (J,J) -> Xst[8..15]
+        {
+            const uint32_t *ph = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_ii));
+            const uint32_t *pv = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_jj)) + C::PANEL_WORDS;
+            for (int e = tid; e < C::PANEL_WORDS; e += C::NTHR) {
+                const int g = e / T, k = e % T;
+                sm.Wst[g * C::TP + k] = __ldcg(ph + e);
+                sm.Xst[(8 + g) * C::TP + k] = __ldcg(pv + e);
+            }
+        }
+        // bulk maxima gathered by the PROD stages (or zero)
+        if (S > 0) {
+            const int16_t *accg = p.acc + (size_t)sidx * T * T;
+            for (int e = tid; e < T * T; e += C::NTHR) sm.val[(e / T) * C::VP + (e % T) + 1] = __ldcg(accg + e);
+        } else {
+            for (int e = tid; e < T * T; e += C::NTHR) sm.val[(e / T) * C::VP + (e % T) + 1] = 0;
+        }
+        // neighbours' edges: right column of (I,J-1) -> val[a][0]; top row of (I+1,J) -> val[T][jj+1];
+        // corner M((I+1)T, JT-1) = top row of (I+1,J-1) at its last column (0 if that tile is below the diagonal)
+        {
+            const uint16_t *eleft = reinterpret_cast<const uint16_t *>(rec_ptr<Q>(p, s_left) + 2 * C::PANEL_WORDS * 4);
+            const uint16_t *ebelow = reinterpret_cast<const uint16_t *>(rec_ptr<Q>(p, s_below) + 2 * C::PANEL_WORDS * 4);
+            if (tid < T) {
+                sm.val[tid * C::VP] = (int16_t)__ldcg(eleft + T + tid);          // right column
+                sm.val[T * C::VP + tid + 1] = (int16_t)__ldcg(ebelow + tid);     // top row
+            }
+            if (tid == T) {
+                int corner = 0;
+                if (dp >= 2) {
+                    const uint16_t *ec = reinterpret_cast<const uint16_t *>(
+                        rec_ptr<Q>(p, si.sbase + tri_index(nt, I + 1, J - 1)) + 2 * C::PANEL_WORDS * 4);
+                    corner = __ldcg(ec + T - 1);
+                }
+                sm.val[T * C::VP] = (int16_t)corner;
+            }
+        }
+        __syncthreads();
+        // late products: the middle blocks whose panels were only finished on the previous step
+        if (dp >= 2) {
+            const int jj = tid % T, rb = tid / T;
+            uint32_t acc[C::RPT];
+#pragma unroll
+            for (int rr = 0; rr < C::RPT; ++rr) acc[rr] = 0;
+            const int K0 = I + 1, K1 = J - 1;
+            load_operands_async<Q>(p, sm, 0, si.sbase + tri_index(nt, I, K0), si.sbase + tri_index(nt, K0, J));
+            if (K1 != K0) {
+                load_operands_async<Q>(p, sm, 1, si.sbase + tri_index(nt, I, K1), si.sbase + tri_index(nt, K1, J));
+                cp_async_wait<1>();
+            } else {
+                cp_async_wait<0>();
+            }
+            __syncthreads();
+            product_accumulate<Q>(sm, 0, acc, jj, rb);
+            if (K1 != K0) {
+                cp_async_wait<0>();
+                __syncthreads();
+                product_accumulate<Q>(sm, 1, acc, jj, rb);
+            }
+#pragma unroll
+            for (int rr = 0; rr < C::RPT; ++rr) {
+                int16_t *cell = sm.val + (rb * C::RPT + rr) * C::VP + jj + 1;
+                *cell = (int16_t)max((int)*cell, (int)(acc[rr] >> C::SH));
+            }
+            __syncthreads();
+        }
+        closure_offdiag<Q>(sm);
+    }
+
+    // ---- publish: row panel, column panel, edges (step a6 output), optional table block, score ----
+    {
+        uint8_t *rec = const_cast<uint8_t *>(rec_ptr<Q>(p, sidx));
+        uint32_t *ph = reinterpret_cast<uint32_t *>(rec);
+        uint32_t *pv = ph + C::PANEL_WORDS;
+        uint16_t *edge = reinterpret_cast<uint16_t *>(rec + 2 * C::PANEL_WORDS * 4);
+        for (int e = tid; e < C::PANEL_WORDS; e += C::NTHR) {
+            const int g = e / T, k = e % T;
+            __stcg(ph + e, sm.Wst[(8 + g) * C::TP + k]);
+            __stcg(pv + e, sm.Xst[g * C::TP + k]);
+        }
+        if (tid < T) {
+            __stcg(edge + tid, (uint16_t)sm.val[tid + 1]);                       // top row  M(I*T, c)
+            __stcg(edge + T + tid, (uint16_t)sm.val[tid * C::VP + T]);           // right column M(r, J*T+T-1)
+        }
+        const int n = si.n;
+        if (p.table_out) {
+            // out[(i-1)*n + (j-1)] = D(i,j) = M(i-1, j): r = i-1 <= n-1, 1 <= c <= n, c >= r+1
+            for (int e = tid; e < T * T; e += C::NTHR) {
+                const int a = e / T, k = e % T;
+                const int r = I * T + a, c = J * T + k;
+                if (r < n && c >= r + 1 && c <= n) {
+                    const int v = sm.val[a * C::VP + k + 1];
+                    if (p.table_dtype == RNA4R_TABLE_INT16) reinterpret_cast<int16_t *>(p.table_out)[(size_t)r * n + c - 1] = (int16_t)v;
+                    else reinterpret_cast<int32_t *>(p.table_out)[(size_t)r * n + c - 1] = v;
+                }
+            }
+        }
+        if (I == 0 && J == n / T && tid == 0)
+            p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release_gpu(p.done + sidx, 1);
+    }
+}
+
+template <int Q>
+__global__ void __launch_bounds__(Cfg<Q>::NTHR) fill_kernel(Params p)
+{
+    using C = Cfg<Q>;
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    Smem<Q> sm(smem_raw);
+    const int tid = threadIdx.x;
+    // table R (reachable quadrant) -> shared memory, once per CTA
+    {
+        const uint4 *src = reinterpret_cast<const uint4 *>(p.tbl);
+        uint4 *dst = reinterpret_cast<uint4 *>(sm.tbl);
+        for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
+        if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
+    }
+    __syncthreads();
+    const int total = p.hdr->total;
+    for (;;) {
+        if (tid == 0) sm.misc[0] = atomicAdd(&p.hdr->counter, 1);
+        __syncthreads();
+        const int tk = sm.misc[0];
+        if (tk >= total) break;
+        const int4 task = p.tasks[tk];
+        const SeqInfo si = p.seqinfo[task.x];
+        const int I = task.y & 0xffff, J = (task.y >> 16) & 0xffff;
+        if (task.z == TASK_PROD) run_prod<Q>(p, sm, si, I, J, task.w);
+        else run_close<Q>(p, sm, si, task.x, I, J);
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side: workspace layout and enqueue
+// ------------------------------------------------------------------------------------------------
+struct HostPlan {
+    size_t tiles, codes, tasks;
+    int max_nt;
+};
+
+static inline HostPlan host_plan(int T, int delta, const int32_t *lens, int count, int n_single)
+{
+    HostPlan h{0, 0, 0, 1};
+    for (int t = 0; t < count; ++t) {
+        const int n = lens ? lens[t] : n_single;
+        const int nt = n / T + 1;
+        h.tiles += (size_t)nt * (nt + 1) / 2;
+        h.codes += (size_t)nt * T;
+        if (nt > h.max_nt) h.max_nt = nt;
+        h.tasks += (size_t)nt * (nt + 1) / 2;
+        for (int dp = 4; dp <= nt - 1; ++dp) h.tasks += (size_t)nstages(dp, delta) * (nt - dp);
+    }
+    return h;
+}
+
+struct WsLayout {
+    size_t zero_bytes;   // prefix that must be zeroed before every fold
+    size_t off_hdr, off_stepC, off_stepP, off_curC, off_curP, off_done, off_accstage;
+    size_t off_seqinfo, off_tasks, off_codes, off_recs, off_acc, total;
+};
+
+static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int count)
+{
+    WsLayout w;
+    size_t off = 0;
+    w.off_hdr = off; off += 256;
+    w.off_stepC = off; off += align_up((size_t)h.max_nt * 4, 256);
+    w.off_stepP = off; off += align_up((size_t)h.max_nt * 4, 256);
+    w.off_curC = off; off += align_up((size_t)h.max_nt * 4, 256);
+    w.off_curP = off; off += align_up((size_t)h.max_nt * 4, 256);
+    w.off_done = off; off += align_up(h.tiles * 4, 256);
+    w.off_accstage = off; off += align_up(h.tiles * 4, 256);
+    w.zero_bytes = off;
+    w.off_seqinfo = off; off += align_up((size_t)count * sizeof(SeqInfo), 256);
+    w.off_tasks = off; off += align_up(h.tasks * sizeof(int4), 256);
+    w.off_codes = off; off += align_up(h.codes, 256);
+    w.off_recs = off; off += align_up(h.tiles * (size_t)rec_bytes, 256);
+    w.off_acc = off; off += align_up(h.tiles * (size_t)T * T * 2, 256);
+    w.total = off;
+    return w;
+}
+
+template <int Q>
+static size_t workspace_bytes_q(int delta, const int32_t *lens, int count, int n_single)
+{
+    using C = Cfg<Q>;
+    const HostPlan h = host_plan(C::T, delta, lens, count, n_single);
+    return ws_layout(C::T, C::REC_BYTES, h, count).total;
+}
+
+template <int Q>
+static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64_t *offsets, const int32_t *lens_host,
+                     int count, int n_single, int32_t *scores, void *table_out, int table_dtype, void *ws, cudaStream_t st)
+{
+    using C = Cfg<Q>;
+    const HostPlan h = host_plan(C::T, delta, lens_host, count, n_single);
+    const WsLayout w = ws_layout(C::T, C::REC_BYTES, h, count);
+    char *base = (char *)ws;
+    Params p;
+    p.seqs = seqs; p.offsets = offsets; p.n_single = n_single; p.count = count; p.max_nt = h.max_nt; p.delta = delta;
+    p.hdr = (PlanHdr *)(base + w.off_hdr);
+    p.stepC = (int *)(base + w.off_stepC); p.stepP = (int *)(base + w.off_stepP);
+    p.curC = (int *)(base + w.off_curC); p.curP = (int *)(base + w.off_curP);
+    p.done = (int *)(base + w.off_done); p.accstage = (int *)(base + w.off_accstage);
+    p.seqinfo = (SeqInfo *)(base + w.off_seqinfo);
+    p.tasks = (int4 *)(base + w.off_tasks);
+    p.codes = (int8_t *)(base + w.off_codes);
+    p.recs = (uint8_t *)(base + w.off_recs);
+    p.acc = (int16_t *)(base + w.off_acc);
+    p.tbl = C::NIBBLE ? ctx->Rc4 : ctx->Rc;
+    p.scores = scores; p.table_out = table_out; p.table_dtype = table_dtype;
+
+    static bool attr_set = false;
+    if (!attr_set) {
+        RNA4R_CUDA(ctx, cudaFuncSetAttribute(fill_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+        attr_set = true;
+    }
+    if (ctx->tiled_blocks_per_sm == 0) {
+        int nb = 0;
+        RNA4R_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fill_kernel<Q>, C::NTHR, C::SMEM_BYTES));
+        if (nb < 1) return RNA4R_ERR_CUDA;
+        ctx->tiled_blocks_per_sm = nb;
+    }
+    int launches = 0;
+    RNA4R_CUDA(ctx, cudaMemsetAsync(ws, 0, w.zero_bytes, st));
+    plan_seq_kernel<Q><<<(count + 127) / 128, 128, 0, st>>>(p); ++launches;
+    plan_scan_kernel<<<1, 32, 0, st>>>(p); ++launches;
+    plan_fill_kernel<Q><<<count * h.max_nt, 64, 0, st>>>(p); ++launches;
+    {
+        const int maxlen = h.max_nt * C::T;
+        dim3 grid((maxlen + 255) / 256, count);
+        encode_kernel<Q><<<grid, 256, 0, st>>>(p); ++launches;
+    }
+    size_t want = h.tasks;
+    int blocks = ctx->sm_count * ctx->tiled_blocks_per_sm;
+    if ((size_t)blocks > want) blocks = (int)want;
+    if (blocks < 1) blocks = 1;
+    fill_kernel<Q><<<blocks, C::NTHR, C::SMEM_BYTES, st>>>(p); ++launches;
+    RNA4R_CUDA(ctx, cudaGetLastError());
+    ctx->last_launches = launches;
+    return RNA4R_OK;
+}
+
+}  // namespace tiled
