@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py -- times the two-vector Four-Russians fold on B200 and prints ONE JSON line.
+
+Workload at N=1: BASELINE.json's headline configuration, configs[2] = "single sequence n=6000,
+i.i.d. uniform {A,C,G,U}, seed 2, q=8" (the paper's largest length; the metric "fold time at
+n=6000 (s) and cell-k-updates/s" is quoted on it).  A step = one whole fold through the C ABI
+(rna4r_fold: encode, plan, persistent wavefront fill with fused vector packing, score) with the
+sequence already resident in HBM; rna4r_prepare (the one-time R-table build, step a2) is timed
+separately and reported as `prepare_ms`.  `e2e` is the same fold through rna4r_fold_host with
+pinned HOST buffers, host<->device copies inside the timed region.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-cpu] [--no-also]
+
+N>1 (torchrun): the single fold does not shard (every cell needs its whole row and column,
+PAPER.md:223) -- "replicas only": each rank folds its own replica, value = N*W / max-rank time.
+
+--impl reference: the oracle (oracle/, plain eq. (1), 1 thread) timed as it stands on a bounded
+sample of the same workload (the first 2000 bases of the same sequence).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+Q = 8
+CFG = "cfg3"
+WORKLOAD = "cfg3: single RNA sequence n=6000, i.i.d. uniform {A,C,G,U}, seed 2, q=8, score only (BASELINE.json configs[2])"
+
+
+def nussinov_updates(n: int) -> int:
+    """W(n) = n(n^2-1)/6 Nussinov-equivalent cell-k-updates (inner-loop steps of eq. (1))."""
+    return n * (n * n - 1) // 6
+
+
+def algorithmic_lookups(n: int, q: int) -> int:
+    """L = sum_d (n-d) floor(d/q): table lookups of the two-vector fill."""
+    d = np.arange(1, n, dtype=np.int64)
+    return int(((n - d) * (d // q)).sum())
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.01):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.sm_max = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, nm in names.items():
+                    if mask & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        return {
+            "sm_mhz": float(np.median(self.samples)) if self.samples else None,
+            "sm_max_mhz": self.sm_max,
+            "reasons": sorted(self.reasons),
+            "samples": len(self.samples),
+        }
+
+
+def cpu_baselines(seq: bytes, q: int):
+    """Oracle as it stands, host cores, bounded sample; plus the serial two-vector build."""
+    import oracle
+    n_s = 3000
+    t0 = time.perf_counter()
+    sc = oracle.nussinov(seq[:n_s])
+    dt = time.perf_counter() - t0
+    base = {
+        "value": nussinov_updates(n_s) / dt, "unit": "cell-k-updates/s", "cores": 1, "kind": "oracle",
+        "sample": f"plain eq.(1) oracle (oracle_nussinov, int32, 1 thread) on the first {n_s} bases of the same sequence: {dt:.2f} s, D(1,{n_s})={sc}",
+    }
+    t0 = time.perf_counter()
+    tv = oracle.two_vector_serial(seq, q)
+    dt2 = time.perf_counter() - t0
+    extra = {
+        "two_vector_serial": {
+            "value": nussinov_updates(len(seq)) / dt2, "unit": "cell-k-updates/s", "cores": 1, "seconds": dt2,
+            "sample": f"Algorithm 1 (PAPER.md:125-187), q={q}, whole n={len(seq)} fold, 1 thread; paper: ~57 s desktop / ~15 s server (PAPER.md:13)",
+            "score": tv["score"],
+        }
+    }
+    return base, extra
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle timed as it stands on a bounded sample per step."""
+    if rank != 0:
+        return
+    import oracle
+    seq = workloads.single_config(CFG)
+    n_s = 2000
+    sample = seq[:n_s]
+    for _ in range(args.warmup):
+        oracle.nussinov(sample)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.nussinov(sample)
+    dt = (time.perf_counter() - t0) / max(args.steps, 1)
+    val = nussinov_updates(n_s) / dt
+    desc = f"plain eq.(1) oracle (oracle_nussinov, 1 thread) on the first {n_s} bases of the cfg3 sequence, one fold per step"
+    print(json.dumps({
+        "impl": "reference", "metric": "cell_k_updates_per_s", "value": val, "unit": "cell-k-updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "q": Q, "n": 6000},
+        "cpu_baseline": {"value": val, "unit": "cell-k-updates/s", "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": "cell-k-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-also", action="store_true", help="skip the extra workloads (cfg2, cfg4 batch, cfg5)")
+    ap.add_argument("--engine", default="tiled", choices=["tiled", "diag"])
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import paper_1307_7820_b200 as pkg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    args.warmup = max(args.warmup, 3)
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    peaks = measured_peaks()
+    seq = workloads.single_config(CFG)
+    n = len(seq)
+    W_updates = nussinov_updates(n)
+    L_lookups = algorithmic_lookups(n, Q)
+
+    # one-time preprocessing (step a2), timed separately
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    r = pkg.Rna4r(Q, local_rank, pkg.ENGINE_TILED if args.engine == "tiled" else pkg.ENGINE_DIAG)
+    torch.cuda.synchronize()
+    prepare_ms = (time.perf_counter() - t0) * 1e3
+    r.enable_kernel_timing(True)
+
+    seq_dev = torch.from_numpy(np.frombuffer(seq, dtype=np.uint8).copy()).cuda()
+    score_dev = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws = r.workspace(r.workspace_bytes_host(np.array([n], dtype=np.int32)))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def one_fold():
+        r.fold(seq_dev, n, score_out=score_dev, workspace=ws, stream=stream)
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        one_fold()
+    torch.cuda.synchronize()
+    score = int(score_dev.item())
+
+    # ---- timed region: K folds, each bracketed by CUDA events on the launching stream; L2 flushed between
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    fill_ms = []
+    launches = 0
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)
+        ev[k][0].record(stream)
+        one_fold()
+        ev[k][1].record(stream)
+        launches += r.last_launch_count()
+        fill_ms.append(r.last_fill_kernel_ms())       # waits for this fold's dominant kernel
+    barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    # keep the GPU busy a little longer so the sampler sees clocks under load even for short runs
+    t_end = time.perf_counter() + 0.25
+    while time.perf_counter() < t_end:
+        one_fold()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * W_updates / (ms_per_step * 1e-3)
+
+    # ---- e2e: host buffers through rna4r_fold_host, copies inside the timed region (wall clock, synchronous call)
+    seq_pinned = torch.from_numpy(np.frombuffer(seq, dtype=np.uint8).copy()).pin_memory()
+    score_pinned = torch.zeros(1, dtype=torch.int32).pin_memory()
+    for _ in range(3):
+        r.fold_host(seq_pinned, workspace=ws, stream=stream, score_host=score_pinned)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        sc_e2e, _ = r.fold_host(seq_pinned, workspace=ws, stream=stream, score_host=score_pinned)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / args.steps
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    assert sc_e2e == score
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the persistent fill kernel)
+    fill_avg_ms = float(np.mean(fill_ms))
+    sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    peak_lookups = sm_count * 32 * peaks["sm_max_mhz"] * 1e6          # one 32-lane shared-memory wavefront / SM / clk
+    ach_lookups = L_lookups / (fill_avg_ms * 1e-3)
+    alg_bytes = n + 4                                                  # read n bases, write one int32 score
+    roofline = {
+        "bound": "smem", "kernel": "tiled::fill_kernel<8>" if args.engine == "tiled" else "diag_fill_kernel (all diagonals)",
+        "achieved": ach_lookups / 1e9, "peak": peak_lookups / 1e9, "unit": "Glookup/s",
+        "frac": ach_lookups / peak_lookups,
+        "traffic": None,
+        "per_unit": "1 table lookup = one 1-byte shared-memory gather (replaces q=8 inner-loop steps); "
+                    f"units per launch L = sum_d (n-d) floor(d/q) = {L_lookups}",
+        "peak_source": f"{sm_count} SMs x 32 lanes x {peaks['sm_max_mhz']:.0f} MHz (max SM clock, MEASURED_PEAKS.json: {peaks['source']})",
+        "kernel_ms": fill_avg_ms, "kernel_share_of_step": fill_avg_ms / ms_per_step,
+        "hbm": {"algorithmic_bytes": alg_bytes, "achieved_gbs": alg_bytes / (fill_avg_ms * 1e-3) / 1e9,
+                "peak_gbs": peaks["hbm_gbs"], "frac": alg_bytes / (fill_avg_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "note": "not the binding roofline: the fold reads n bytes and writes 4"},
+    }
+    # optional ncu-measured DRAM traffic of the same kernel (profiles/), per launch
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as f:
+                roofline["traffic"] = json.load(f).get("cfg3_fill_kernel_dram_bytes")
+        except Exception:
+            pass
+
+    out = {
+        "metric": "cell_k_updates_per_s", "value": value, "unit": "cell-k-updates/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "fold_time_s": ms_per_step * 1e-3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "n": n, "q": Q, "engine": args.engine, "score": score,
+                   "l2": "flushed between steps (256 MB write)", "prepare": "rna4r_prepare timed separately (prepare_ms)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "prepare_ms": prepare_ms,
+        "clocks": clocks,
+        "e2e": {"value": world * W_updates / e2e_s, "unit": "cell-k-updates/s", "seconds_per_fold": e2e_s,
+                "h2d_bytes_per_step": n, "d2h_bytes_per_step": 4},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "paper_context": {"tesla_c2070_s": 2.50, "geforce_gtx550ti_s": 4.97, "cite": "PAPER.md:345"},
+    }
+
+    if not args.no_also and world == 1:
+        out["also"] = also_workloads(pkg, torch, r, flush)
+    if not args.no_cpu and world == 1:
+        base, extra = cpu_baselines(seq, Q)
+        out["cpu_baseline"] = base
+        out["cpu_baselines_extra"] = extra
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def also_workloads(pkg, torch, r8, flush):
+    """Device-timed numbers for the other configs (parity cases; context beside the headline)."""
+    res = {}
+
+    def time_call(fn, reps):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            flush.fill_(3)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.median(ts))
+
+    # cfg2
+    s = workloads.single_config("cfg2")
+    d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()
+    ms = time_call(lambda: r8.fold(d), 10)
+    res["cfg2_n2000_q8"] = {"ms": ms, "cell_k_updates_per_s": nussinov_updates(len(s)) / (ms * 1e-3)}
+    # cfg4 batch
+    seqs, lens = workloads.gc_rich_batch()
+    flat, offsets, lens32 = workloads.pack_batch(seqs)
+    fd, od = torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda()
+    wsb = torch.empty(r8.workspace_bytes_batch(lens32), dtype=torch.uint8, device="cuda")
+    sc = torch.empty(len(lens32), dtype=torch.int32, device="cuda")
+    ms = time_call(lambda: r8.fold_batch(fd, od, lens32, scores_out=sc, workspace=wsb), 10)
+    wtot = int(sum(nussinov_updates(int(x)) for x in lens32))
+    ltot = int(sum(algorithmic_lookups(int(x), 8) for x in lens32))
+    res["cfg4_batch1024_q8"] = {"ms": ms, "cell_k_updates_per_s": wtot / (ms * 1e-3), "fill_kernel_ms": r8.last_fill_kernel_ms(),
+                               "lookups": ltot, "sum_scores": int(sc.sum().item())}
+    del wsb
+    # cfg5
+    s = workloads.single_config("cfg5")
+    d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()
+    for q in (8, 10):
+        rr = r8 if q == 8 else pkg.Rna4r(10, 0)
+        rr.enable_kernel_timing(True)
+        ms = time_call(lambda: rr.fold(d), 3)
+        res[f"cfg5_n16384_q{q}"] = {"ms": ms, "cell_k_updates_per_s": nussinov_updates(len(s)) / (ms * 1e-3),
+                                    "fill_kernel_ms": rr.last_fill_kernel_ms(), "lookups": algorithmic_lookups(len(s), q)}
+    return res
+
+
+if __name__ == "__main__":
+    main()

@@ -161,6 +161,16 @@ int rna4r_fold_batch_host(rna4r_ctx *ctx, const uint8_t *seqs_host, const int32_
 /* Number of kernel launches the most recent fold call enqueued (for accounting), or < 0. */
 int rna4r_last_launch_count(const rna4r_ctx *ctx);
 
+/*
+ * Kernel timing for roofline accounting.  With timing enabled (on != 0) every fold call records a pair
+ * of CUDA events on the launching stream around its dominant kernel -- the persistent fill kernel of
+ * the TILED engine, or the whole sequence of per-diagonal launches of the DIAG engine (for a DIAG
+ * batch: the last sequence).  rna4r_last_fill_kernel_ms waits for the second event and writes the
+ * elapsed milliseconds to *ms_host.  Errors: CONTEXT, NULL, CUDA (also when nothing was recorded).
+ */
+int rna4r_enable_kernel_timing(rna4r_ctx *ctx, int on);
+int rna4r_last_fill_kernel_ms(rna4r_ctx *ctx, float *ms_host);
+
 /* cudaError_t of the most recent failing CUDA call on this context (0 if none). */
 int rna4r_last_cuda_error(const rna4r_ctx *ctx);
 

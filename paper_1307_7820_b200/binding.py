@@ -59,6 +59,8 @@ def load():
     L.rna4r_fold_batch.argtypes = [vp, u8p, i64p, i32p, ctypes.c_int, i32p, vp, ctypes.c_size_t, vp]
     L.rna4r_fold_host.argtypes = [vp, u8p, ctypes.c_int, i32p, vp, ctypes.c_int, vp, ctypes.c_size_t, vp]
     L.rna4r_fold_batch_host.argtypes = [vp, u8p, i32p, ctypes.c_int, i32p, vp, ctypes.c_size_t, vp]
+    L.rna4r_enable_kernel_timing.argtypes = [vp, ctypes.c_int]
+    L.rna4r_last_fill_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     L.rna4r_last_launch_count.argtypes = [vp]
     L.rna4r_last_cuda_error.argtypes = [vp]
     _lib = L
@@ -126,6 +128,14 @@ class Rna4r:
         out = np.empty((side, side), dtype=np.uint8)
         _check(self.lib.rna4r_table_to_host(self.h, out.ctypes.data, compact), "rna4r_table_to_host")
         return out
+
+    def enable_kernel_timing(self, on: bool = True):
+        _check(self.lib.rna4r_enable_kernel_timing(self.h, int(on)), "rna4r_enable_kernel_timing")
+
+    def last_fill_kernel_ms(self) -> float:
+        ms = ctypes.c_float(0)
+        _check(self.lib.rna4r_last_fill_kernel_ms(self.h, ctypes.byref(ms)), "rna4r_last_fill_kernel_ms")
+        return float(ms.value)
 
     def last_launch_count(self) -> int:
         return self.lib.rna4r_last_launch_count(self.h)

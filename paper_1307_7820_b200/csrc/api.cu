@@ -102,6 +102,7 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     ctx->sm_count = prop.multiProcessorCount;
     ctx->R = ctx->Rc = ctx->Rc4 = nullptr;
     ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0;
+    ctx->timing = 0; ctx->timing_valid = 0; ctx->ev0 = ctx->ev1 = nullptr;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t N = (size_t)1 << q, M = (size_t)1 << (q - 1);
     auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4); delete ctx; return RNA4R_ERR_CUDA; };
@@ -131,6 +132,8 @@ int rna4r_destroy(rna4r_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     ctx->magic = 0;
     delete ctx;
     return RNA4R_OK;
@@ -151,6 +154,29 @@ int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact)
     RNA4R_CUDA(ctx, cudaDeviceSynchronize());
     const size_t side = (size_t)1 << (compact ? ctx->q - 1 : ctx->q);
     RNA4R_CUDA(ctx, cudaMemcpy(dst_host, compact ? ctx->Rc : ctx->R, side * side, cudaMemcpyDeviceToHost));
+    return RNA4R_OK;
+}
+
+int rna4r_enable_kernel_timing(rna4r_ctx *ctx, int on)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (on && !ctx->ev0) {
+        RNA4R_CUDA(ctx, cudaEventCreate(&ctx->ev0));
+        RNA4R_CUDA(ctx, cudaEventCreate(&ctx->ev1));
+    }
+    ctx->timing = on ? 1 : 0;
+    ctx->timing_valid = 0;
+    return RNA4R_OK;
+}
+
+int rna4r_last_fill_kernel_ms(rna4r_ctx *ctx, float *ms_host)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (!ms_host) return RNA4R_ERR_NULL;
+    if (!ctx->timing_valid) { ctx->last_cuda_error = 0; return RNA4R_ERR_CUDA; }
+    RNA4R_CUDA(ctx, cudaEventSynchronize(ctx->ev1));
+    RNA4R_CUDA(ctx, cudaEventElapsedTime(ms_host, ctx->ev0, ctx->ev1));
     return RNA4R_OK;
 }
 

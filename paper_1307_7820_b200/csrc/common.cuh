@@ -17,6 +17,9 @@ struct rna4r_ctx {
     int last_launches;
     int last_cuda_error;
     int tiled_blocks_per_sm; // occupancy of the tiled fill kernel for this q (0 = not queried yet)
+    int timing;              // record events around the dominant kernel
+    int timing_valid;
+    cudaEvent_t ev0, ev1;
 };
 static const uint32_t RNA4R_MAGIC = 0x52344e41u;
 

@@ -127,11 +127,13 @@ static int diag_fold_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int3
         ++launches;
     }
     const int q = ctx->q;
+    if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
     for (int d = 1; d <= n - 1; ++d) {
         const int cells = n - d;
         diag_fill_kernel<<<(cells + 127) / 128, 128, 0, st>>>(n, q, d, w.codes, ctx->R, w.Dd, w.Hd, w.Vd, w.hrun, w.vrun);
         ++launches;
     }
+    if (ctx->timing) { RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev1, st)); ctx->timing_valid = 1; }
     if (n == 0) {
         RNA4R_CUDA(ctx, cudaMemsetAsync(score_dev, 0, sizeof(int32_t), st));
     } else {

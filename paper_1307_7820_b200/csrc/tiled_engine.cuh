@@ -766,7 +766,9 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     int blocks = ctx->sm_count * ctx->tiled_blocks_per_sm;
     if ((size_t)blocks > want) blocks = (int)want;
     if (blocks < 1) blocks = 1;
+    if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
     fill_kernel<Q><<<blocks, C::NTHR, C::SMEM_BYTES, st>>>(p); ++launches;
+    if (ctx->timing) { RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev1, st)); ctx->timing_valid = 1; }
     RNA4R_CUDA(ctx, cudaGetLastError());
     ctx->last_launches = launches;
     return RNA4R_OK;
