@@ -172,6 +172,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-also", action="store_true", help="skip the extra workloads (cfg2, cfg4 batch, cfg5)")
+    ap.add_argument("--profile", action="store_true", help="short run for ncu: no e2e leg, no tail loop, no extras")
     ap.add_argument("--engine", default="tiled", choices=["tiled", "diag"])
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -245,7 +246,7 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
     # keep the GPU busy a little longer so the sampler sees clocks under load even for short runs
-    t_end = time.perf_counter() + 0.25
+    t_end = time.perf_counter() + (0.0 if args.profile else 0.25)
     while time.perf_counter() < t_end:
         one_fold()
     torch.cuda.synchronize()
@@ -261,14 +262,14 @@ def main():
     # ---- e2e: host buffers through rna4r_fold_host, copies inside the timed region (wall clock, synchronous call)
     seq_pinned = torch.from_numpy(np.frombuffer(seq, dtype=np.uint8).copy()).pin_memory()
     score_pinned = torch.zeros(1, dtype=torch.int32).pin_memory()
-    for _ in range(3):
+    for _ in range(0 if args.profile else 3):
         r.fold_host(seq_pinned, workspace=ws, stream=stream, score_host=score_pinned)
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(1 if args.profile else args.steps):
         sc_e2e, _ = r.fold_host(seq_pinned, workspace=ws, stream=stream, score_host=score_pinned)
     torch.cuda.synchronize()
-    e2e_s = (time.perf_counter() - t0) / args.steps
+    e2e_s = (time.perf_counter() - t0) / (1 if args.profile else args.steps)
     if dist is not None:
         t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -326,6 +327,8 @@ def main():
         "paper_context": {"tesla_c2070_s": 2.50, "geforce_gtx550ti_s": 4.97, "cite": "PAPER.md:345"},
     }
 
+    if args.profile:
+        args.no_also = args.no_cpu = True
     if not args.no_also and world == 1:
         out["also"] = also_workloads(pkg, torch, r, flush)
     if not args.no_cpu and world == 1:

@@ -171,6 +171,18 @@ int rna4r_last_launch_count(const rna4r_ctx *ctx);
 int rna4r_enable_kernel_timing(rna4r_ctx *ctx, int on);
 int rna4r_last_fill_kernel_ms(rna4r_ctx *ctx, float *ms_host);
 
+/*
+ * Wavefront trace (TILED engine; a profiling aid for the per-diagonal latency of step a7).  With
+ * max_tiles > 0 the context allocates max_tiles * 64 bytes; every closure task of a later fold then
+ * writes eight uint64 for its super-tile (index = order of the triangular enumeration, row-major
+ * I <= J): %globaltimer ns at [0] task claimed, [1] dependencies met, [2] operands loaded, [3] late
+ * products done, [4] in-tile wavefront done, [5] published; [6] = I << 32 | J; [7] unused.
+ * max_tiles = 0 frees the buffer and switches tracing off.  rna4r_trace_to_host synchronises the
+ * device and copies `tiles` records to HOST memory.  Errors: CONTEXT, NULL, BAD_N, CUDA.
+ */
+int rna4r_set_trace(rna4r_ctx *ctx, int max_tiles);
+int rna4r_trace_to_host(rna4r_ctx *ctx, uint64_t *dst_host, int tiles);
+
 /* cudaError_t of the most recent failing CUDA call on this context (0 if none). */
 int rna4r_last_cuda_error(const rna4r_ctx *ctx);
 

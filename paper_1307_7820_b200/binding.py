@@ -61,6 +61,8 @@ def load():
     L.rna4r_fold_batch_host.argtypes = [vp, u8p, i32p, ctypes.c_int, i32p, vp, ctypes.c_size_t, vp]
     L.rna4r_enable_kernel_timing.argtypes = [vp, ctypes.c_int]
     L.rna4r_last_fill_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.rna4r_set_trace.argtypes = [vp, ctypes.c_int]
+    L.rna4r_trace_to_host.argtypes = [vp, vp, ctypes.c_int]
     L.rna4r_last_launch_count.argtypes = [vp]
     L.rna4r_last_cuda_error.argtypes = [vp]
     _lib = L
@@ -136,6 +138,14 @@ class Rna4r:
         ms = ctypes.c_float(0)
         _check(self.lib.rna4r_last_fill_kernel_ms(self.h, ctypes.byref(ms)), "rna4r_last_fill_kernel_ms")
         return float(ms.value)
+
+    def set_trace(self, max_tiles: int):
+        _check(self.lib.rna4r_set_trace(self.h, int(max_tiles)), "rna4r_set_trace")
+
+    def trace(self, tiles: int) -> np.ndarray:
+        out = np.zeros((tiles, 8), dtype=np.uint64)
+        _check(self.lib.rna4r_trace_to_host(self.h, out.ctypes.data, tiles), "rna4r_trace_to_host")
+        return out
 
     def last_launch_count(self) -> int:
         return self.lib.rna4r_last_launch_count(self.h)

@@ -103,6 +103,7 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     ctx->R = ctx->Rc = ctx->Rc4 = nullptr;
     ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0;
     ctx->timing = 0; ctx->timing_valid = 0; ctx->ev0 = ctx->ev1 = nullptr;
+    ctx->trace = nullptr; ctx->trace_tiles = 0;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t N = (size_t)1 << q, M = (size_t)1 << (q - 1);
     auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4); delete ctx; return RNA4R_ERR_CUDA; };
@@ -132,6 +133,7 @@ int rna4r_destroy(rna4r_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4);
+    cudaFree(ctx->trace);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     ctx->magic = 0;
@@ -154,6 +156,32 @@ int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact)
     RNA4R_CUDA(ctx, cudaDeviceSynchronize());
     const size_t side = (size_t)1 << (compact ? ctx->q - 1 : ctx->q);
     RNA4R_CUDA(ctx, cudaMemcpy(dst_host, compact ? ctx->Rc : ctx->R, side * side, cudaMemcpyDeviceToHost));
+    return RNA4R_OK;
+}
+
+int rna4r_set_trace(rna4r_ctx *ctx, int max_tiles)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    RNA4R_CUDA(ctx, cudaDeviceSynchronize());
+    cudaFree(ctx->trace);
+    ctx->trace = nullptr; ctx->trace_tiles = 0;
+    if (max_tiles > 0) {
+        RNA4R_CUDA(ctx, cudaMalloc(&ctx->trace, (size_t)max_tiles * 64));
+        RNA4R_CUDA(ctx, cudaMemset(ctx->trace, 0, (size_t)max_tiles * 64));
+        ctx->trace_tiles = max_tiles;
+    }
+    return RNA4R_OK;
+}
+
+int rna4r_trace_to_host(rna4r_ctx *ctx, uint64_t *dst_host, int tiles)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (!dst_host) return RNA4R_ERR_NULL;
+    if (!ctx->trace || tiles < 0 || tiles > ctx->trace_tiles) return RNA4R_ERR_BAD_N;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    RNA4R_CUDA(ctx, cudaDeviceSynchronize());
+    RNA4R_CUDA(ctx, cudaMemcpy(dst_host, ctx->trace, (size_t)tiles * 64, cudaMemcpyDeviceToHost));
     return RNA4R_OK;
 }
 

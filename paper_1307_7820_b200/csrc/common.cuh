@@ -20,6 +20,8 @@ struct rna4r_ctx {
     int timing;              // record events around the dominant kernel
     int timing_valid;
     cudaEvent_t ev0, ev1;
+    unsigned long long *trace;   // optional per-super-tile phase stamps (rna4r_set_trace)
+    int trace_tiles;
 };
 static const uint32_t RNA4R_MAGIC = 0x52344e41u;
 
@@ -48,6 +50,12 @@ __device__ __forceinline__ int rna4r_base_code(uint8_t c)
 // b(x,y) of eq. (1): A-U and C-G pair; code 4 (padding / invalid) pairs with nothing
 __device__ __forceinline__ int rna4r_pair(int x, int y) { return (x + y == 3) ? 1 : 0; }
 
+__device__ __forceinline__ unsigned long long global_timer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ int ld_acquire_gpu(const int *p)
 {
     int v;

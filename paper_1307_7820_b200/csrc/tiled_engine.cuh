@@ -29,6 +29,7 @@
 // barrier per diagonal ("Synchronize with other processes").
 #pragma once
 #include "common.cuh"
+#include <cstdlib>
 
 namespace tiled {
 
@@ -47,7 +48,7 @@ struct Cfg {
     static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
     static constexpr int REC_BYTES = 2 * PANEL_WORDS * 4 + 2 * T * 2;   // PH, PV, top row, right column
     static constexpr size_t SMEM_BYTES =
-        (size_t)((TBL_BYTES + 15) / 16 * 16) + 2 * 16 * TP * 4 + 2 * T * 4 + (size_t)(T + 1) * VP * 2 + 2 * 2 * PANEL_WORDS * 4 + 2 * T + 64;
+        (size_t)((TBL_BYTES + 15) / 16 * 16) + 2 * 16 * TP * 4 + (size_t)(T + 1) * VP * 2 + 2 * 2 * PANEL_WORDS * 4 + 2 * T + 64 + (size_t)(Q + 1) * VP * 2;
 };
 
 struct SeqInfo {
@@ -94,6 +95,8 @@ struct Params {
     int32_t *scores;
     void *table_out;
     int table_dtype;
+    unsigned long long *trace;   // NULL, or [tiles][8] phase stamps (ns) of the CLOSE tasks
+    int trace_tiles;
 };
 
 __host__ __device__ inline int nstages(int dp, int delta)
@@ -198,8 +201,6 @@ struct Smem {
     uint8_t *tbl;        // compact table Rc
     uint32_t *Wst;       // [16][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own)
     uint32_t *Xst;       // [16][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static)
-    uint32_t *Wp;        // [T] running (partial) row word of the group being filled
-    uint32_t *Xp;        // [T] running (partial) column word
     int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
     uint32_t *stg;       // [2][2][PANEL_WORDS] product operands, double buffered: [buf][0]=PH, [buf][1]=PV
     int8_t *codeR;       // [T] codes of the rows
@@ -211,8 +212,6 @@ struct Smem {
         tbl = p; p += (C::TBL_BYTES + 15) / 16 * 16;
         Wst = (uint32_t *)p; p += 16 * C::TP * 4;
         Xst = (uint32_t *)p; p += 16 * C::TP * 4;
-        Wp = (uint32_t *)p; p += C::T * 4;
-        Xp = (uint32_t *)p; p += C::T * 4;
         stg = (uint32_t *)p; p += 2 * 2 * C::PANEL_WORDS * 4;
         val = (int16_t *)p; p += (C::T + 1) * C::VP * 2;
         codeR = (int8_t *)p; p += C::T;
@@ -372,117 +371,263 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
     if (tid == 0) st_release_gpu(p.accstage + sidx, S - s);
 }
 
-// ---- closure of an off-diagonal super-tile: 2T-1 anti-diagonal steps, 4 threads per cell ----
+// ------------------------------------------------------------------------------------------------
+// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA)
+//
+// The super-tile is 8 x 8 q-tiles of Q x Q cells; q-tile (A,B) = rows A*Q.., columns B*Q...  q-tiles
+// with equal u = (7-A)+B are independent and are done together (a "macro-step"), in two phases:
+//   P  (all warps, no dependency): every cell of the q-tile takes the maximum over the FULL groups
+//      that lie inside the super-tile's own blocks -- groups x in (A,7] of block I (row words of
+//      (I,I), column words of the q-tiles below, already final) and groups 8..8+B-1 of block J (row
+//      words of the q-tiles to the left, column words of (J,J)).
+//   C  (one lane per column of the q-tile, Q lanes per q-tile): the 2Q-1 anti-diagonal steps
+//       inside the q-tile.  A lane walks its column bottom-up; the running row word
+//      and the neighbour values travel lane to lane by shuffles, the running column word stays in a
+//      register, so a cell-step costs no CTA barrier.  The paper's two residual loops
+//       are the two MASKED lookups: head = (row word of (I,I), running column
+//      word), tail = (running row word, column word of (J,J)).
+// ------------------------------------------------------------------------------------------------
 template <int Q>
-__device__ void closure_offdiag(const Smem<Q> &sm)
+__device__ __forceinline__ uint32_t lookup_cand(const Smem<Q> &sm, uint32_t W, uint32_t X)
+{
+    const uint32_t S = W + X;
+    return (S >> Cfg<Q>::SH) + lookup<Q>(sm.tbl, S & Cfg<Q>::IDXMASK);
+}
+
+// P phase for q-tile (A,B), executed by one warp.  Word-array indices [x0,x1) and [y0,y1).
+template <int Q>
+__device__ __forceinline__ void qtile_products(const Smem<Q> &sm, int A, int B, int x0, int x1, int y0, int y1, int lane)
 {
     using C = Cfg<Q>;
-    constexpr int T = C::T;
-    const int tid = threadIdx.x;
-    const int jj = tid >> 2, part = tid & 3;
-    const int gj = jj / Q, pj = jj % Q;
-    const int x = jj + 1;
-    for (int s = 0; s < 2 * T - 1; ++s) {
-        const int a = T - 1 - (s - jj);
-        const bool active = (a >= 0) && (a < T);
-        uint32_t best = 0;
-        int ga = 0, pa = 0;
-        if (active) {
-            ga = a / Q; pa = a % Q;
+    constexpr int CPL = (Q * Q + 31) / 32;     // cells per lane
+    int row[CPL], col[CPL];
+    uint32_t best[CPL];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int vg = part + 4 * e;
-                uint32_t W, X;
-                bool ok;
-                if (vg < 8) {        // groups of block I: row words of (I,I), column words of this tile (below a)
-                    ok = (vg > ga) || (vg == ga && pa != Q - 1);
-                    W = sm.Wst[vg * C::TP + a];
-                    X = (vg == ga) ? sm.Xp[jj] : sm.Xst[vg * C::TP + jj];
-                } else {             // groups of block J: row words of this tile (left of jj), column words of (J,J)
-                    const int g2 = vg - 8;
-                    ok = (g2 < gj) || (g2 == gj && pj != 0);
-                    X = sm.Xst[vg * C::TP + jj];
-                    W = (g2 == gj) ? sm.Wp[a] : sm.Wst[vg * C::TP + a];
-                }
-                if (ok) {
-                    const uint32_t S = W + X;
-                    const uint32_t rv = lookup<Q>(sm.tbl, S & C::IDXMASK);
-                    best = max(best, (S >> C::SH) + rv);
-                }
-            }
-        }
-        best = max(best, __shfl_xor_sync(0xffffffffu, best, 1));
-        best = max(best, __shfl_xor_sync(0xffffffffu, best, 2));
-        if (active && part == 0) {
-            int16_t *vrow = sm.val + a * C::VP;
-            const int cur = vrow[x];                                                  // bulk maximum
-            const int dg = vrow[C::VP + x - 1] + rna4r_pair(sm.codeR[a], sm.codeC[jj]);   // b + M(r+1,c-1)
-            const int v = max(max(cur, dg), (int)best);
-            vrow[x] = (int16_t)v;
-            const int left = vrow[x - 1], below = vrow[C::VP + x];
-            // step a6: append the horizontal bit to the row word, the vertical bit to the column word
-            const uint32_t wp = (pj == 0) ? ((uint32_t)v << C::SH)
-                                          : (sm.Wp[a] | ((uint32_t)(v - left) << (C::HB + pj - 1)));
-            sm.Wp[a] = wp;
-            if (pj == Q - 1) sm.Wst[(8 + gj) * C::TP + a] = wp;
-            const uint32_t xp = (pa == Q - 1) ? ((uint32_t)v << C::SH)
-                                              : ((sm.Xp[jj] & C::IDXMASK) | ((uint32_t)(v - below) << pa) | ((uint32_t)v << C::SH));
-            sm.Xp[jj] = xp;
-            if (pa == 0) sm.Xst[ga * C::TP + jj] = xp;
-        }
-        __syncthreads();
+    for (int c = 0; c < CPL; ++c) {
+        int e = lane + 32 * c;
+        if (e >= Q * Q) e = Q * Q - 1;           // surplus lanes redo the last cell (same value, benign)
+        row[c] = A * Q + e / Q;
+        col[c] = B * Q + e % Q;
+        best[c] = 0;
+    }
+#pragma unroll 2
+    for (int x = x0; x < x1; ++x) {
+#pragma unroll
+        for (int c = 0; c < CPL; ++c)
+            best[c] = max(best[c], lookup_cand<Q>(sm, sm.Wst[x * C::TP + row[c]], sm.Xst[x * C::TP + col[c]]));
+    }
+#pragma unroll 2
+    for (int y = y0; y < y1; ++y) {
+#pragma unroll
+        for (int c = 0; c < CPL; ++c)
+            best[c] = max(best[c], lookup_cand<Q>(sm, sm.Wst[y * C::TP + row[c]], sm.Xst[y * C::TP + col[c]]));
+    }
+#pragma unroll
+    for (int c = 0; c < CPL; ++c) {
+        int16_t *cell = sm.val + row[c] * C::VP + col[c] + 1;
+        const int cur = *cell;
+        if ((int)best[c] > cur && lane + 32 * c < Q * Q) *cell = (int16_t)best[c];
     }
 }
 
-// ---- closure of a diagonal super-tile (I == J): cells with c <= r+1 are 0; steps s = jj - a ----
+// C phase for q-tile (A,B): lane b (0..Q-1 of its group) owns column b and walks it bottom-up, one
+// cell per step; lane b works one row below lane b-1, so row data flows lane to lane by shuffles.
+// `have` = this lane group has a q-tile.  hg / tg: word-array rows with the head row words / tail
+// column words.
+//
+// Critical-path split.  Of all candidates of cell (a,b) only two depend on the previous step:
+//   left  = v(a,b-1)  (tail split t = c-1: M(r,c-1) + M(c-1,c), M(c-1,c) = 0)
+//   below = v(a+1,b)  (head split t = r+1: M(r,r+1) + M(r+1,c), M(r,r+1) = 0).
+// Everything else -- the bulk maximum, b + D(i+1,j-1), the head lookup over rows >= a+2 and the tail
+// lookup over columns <= b-2 -- is known one step earlier and is folded into OLDX during the previous
+// step.  So the dependent chain of a step is  shuffle -> max -> max.
+//
+// DIAGQ: the q-tile lies on the main diagonal (A == B of a diagonal super-tile): cells with b-a <= 1
+// are 0, rows start at b == a, and head and tail merge into one lookup with both words running.
+template <int Q, bool DIAGQ>
+__device__ __forceinline__ void qtile_closure(const Smem<Q> &sm, bool have, int A, int B, int hg, int tg, bool mirror,
+                                              int lane, int b)
+{
+    using C = Cfg<Q>;
+    const int row0 = A * Q, col = B * Q + b, x = col + 1;
+    const int src1 = (b > 0) ? lane - 1 : lane, src2 = (b > 1) ? lane - 2 : lane;
+    uint32_t Xtail = 0, pm = 0;
+    if (have) {
+        Xtail = sm.Xst[tg * C::TP + col];
+        const int cc = sm.codeC[col];
+#pragma unroll
+        for (int a = 0; a < Q; ++a) pm |= (uint32_t)rna4r_pair(sm.codeR[row0 + a], cc) << a;
+    }
+    uint32_t Xp = 0;        // running column word: rows below the current cell
+    uint32_t outword = 0;   // row word of my last cell's row, my cell included
+    int outv = 0;           // my last value
+    int oldx = 0;           // OLDX of my next cell
+#pragma unroll
+    for (int k = (DIAGQ ? Q - 1 : -1); k < 2 * Q - 1; ++k) {
+        const int L = __shfl_sync(0xffffffffu, outv, src1);                 // v(a, b-1)
+        const uint32_t rw1 = __shfl_sync(0xffffffffu, outword, src1);       // row a,   columns <= b-1
+        const uint32_t rw2 = __shfl_sync(0xffffffffu, outword, src2);       // row a-1, columns <= b-2
+        const int a = Q - 1 - k + b;
+        if (have && a >= 0 && a <= Q) {
+            const int row = row0 + a;
+            int16_t *vrow = sm.val + row * C::VP;
+            int v;
+            if (a < Q) {
+                v = max(oldx, outv);                                        // OLDX, below
+                if (b > 0) v = max(v, L);                                   // left
+                if (DIAGQ && b - a <= 1) v = 0;
+                vrow[x] = (int16_t)v;
+                // step a6: append the horizontal difference bit to the row word
+                const uint32_t myrow = (b == 0 || (DIAGQ && b == a)) ? ((uint32_t)v << C::SH)
+                                                                      : (rw1 | ((uint32_t)(v - L) << (C::HB + b - 1)));
+                outword = myrow;
+                if (b == Q - 1) {
+                    sm.Wst[(8 + B) * C::TP + row] = myrow;
+                    if (mirror) sm.Wst[B * C::TP + row] = myrow;
+                }
+            } else {
+                v = vrow[x];                                                // the cell below the q-tile
+            }
+            if (a >= 1) {                                                   // OLDX of cell (a-1, b)
+                int o = vrow[x - C::VP];                                    // bulk + P-phase maximum
+                const int dgv = (b == 0 || a == Q) ? (int)vrow[x - 1] : L;  // D(i+1,j-1) = v(a, b-1)
+                o = max(o, dgv + (int)((pm >> (a - 1)) & 1u));              // + b(S_i,S_j)
+                if (DIAGQ) {
+                    if (b >= 2) o = max(o, (int)lookup_cand<Q>(sm, rw2, Xp));
+                } else {
+                    if (a <= Q - 2) o = max(o, (int)lookup_cand<Q>(sm, sm.Wst[hg * C::TP + row - 1], Xp));   // head, rows >= a+1
+                    if (b >= 2) o = max(o, (int)lookup_cand<Q>(sm, rw2, Xtail));                             // tail, cols <= b-2
+                }
+                oldx = o;
+            }
+            if (a < Q) {
+                // step a6: append the vertical difference bit to the column word (now rows >= a)
+                Xp = (a == Q - 1) ? ((uint32_t)v << C::SH)
+                                  : ((Xp & C::IDXMASK) | ((uint32_t)(v - outv) << a) | ((uint32_t)v << C::SH));
+                if (a == 0) {
+                    sm.Xst[A * C::TP + col] = Xp;
+                    if (mirror) sm.Xst[(8 + A) * C::TP + col] = Xp;
+                }
+            }
+            outv = v;
+        }
+    }
+}
+
+// Branch-free C phase for the q-tiles of an off-diagonal super-tile (the hot variant of
+// qtile_closure<Q,false>; same recurrence, same fresh/old split).  Every lane group runs a q-tile
+// (surplus groups redo the last one: identical values, benign), every lane runs every step, and
+//   * outside its window (steps b-1 .. b+Q-1) a lane computes don't-care values and stores nothing;
+//   * a lookup whose operand does not exist is fed a zero word, which makes it a valid lower bound:
+//     W = 0 gives M(gq,c) <= M(r,c), X = 0 gives max of the row run <= M(r,c) (Lemma 1 monotonicity);
+//   * all shared-memory addresses are affine in the step index, so the unrolled steps use immediate
+//     offsets (out-of-window loads land in the padded neighbourhood of the arrays and are ignored).
+template <int Q>
+__device__ __forceinline__ void qtile_closure_fast(const Smem<Q> &sm, int A, int B, int lane, int b)
+{
+    using C = Cfg<Q>;
+    const int row0 = A * Q, col = B * Q + b, x = col + 1;
+    const int src1 = (b > 0) ? lane - 1 : lane, src2 = (b > 1) ? lane - 2 : lane;
+    const uint32_t Xtail = sm.Xst[(8 + B) * C::TP + col];
+    uint32_t pm = 0;
+    {
+        const int cc = sm.codeC[col];
+#pragma unroll
+        for (int a = 0; a < Q; ++a) pm |= (uint32_t)rna4r_pair(sm.codeR[row0 + a], cc) << (a + 1);   // bit a+1 <-> row a
+    }
+    // lane-affine bases: at step k the lane is on row  a = Q-1-k+b
+    int16_t *vbase = sm.val + (row0 + Q - 1 + b) * C::VP + x;           // vbase[-k*VP] = val[row][x]
+    const uint32_t *wbase = sm.Wst + A * C::TP + row0 + Q - 2 + b;      // wbase[-k]    = Wst[A][row-1]
+    uint32_t *wout = sm.Wst + (8 + B) * C::TP + row0 + Q - 1 + b;       // wout[-k]     = Wst[8+B][row]
+    const uint32_t rw2mask = (b >= 2) ? 0xffffffffu : 0u;
+    const bool lastcol = (b == Q - 1), firstcol = (b == 0);
+    const int shb = C::HB + b - 1;                                      // position of my horizontal bit
+    uint32_t Xp = 0, outword = 0;
+    int outv = 0, oldx = 0;
+#pragma unroll
+    for (int k = -1; k < 2 * Q - 1; ++k) {
+        const int L = __shfl_sync(0xffffffffu, outv, src1);                 // v(a, b-1)
+        const uint32_t rw1 = __shfl_sync(0xffffffffu, outword, src1);       // row a,   columns <= b-1
+        const uint32_t rw2 = __shfl_sync(0xffffffffu, outword, src2) & rw2mask;   // row a-1, columns <= b-2
+        const int a = Q - 1 - k + b;
+        const bool in = (unsigned)a < (unsigned)Q;
+        int v = max(max(oldx, outv), L);                                    // OLDX, below, left
+        if (a == Q) v = vbase[-k * C::VP];                                  // pre-step: the cell below the q-tile
+        if (in) vbase[-k * C::VP] = (int16_t)v;
+        // step a6, horizontal: my row word = neighbour's word | my difference bit
+        const uint32_t myrow = firstcol ? ((uint32_t)v << C::SH) : (rw1 | ((uint32_t)(v - L) << shb));
+        outword = myrow;
+        if (in && lastcol) wout[-k] = myrow;
+        // OLDX of the next cell (a-1, b)
+        const int dgv = (firstcol || a == Q) ? (int)vbase[-k * C::VP - 1] : L;      // D(i+1,j-1)
+        int o = max((int)vbase[-(k + 1) * C::VP], dgv + (int)((pm >> (a & 31)) & 1u));
+        o = max(o, (int)lookup_cand<Q>(sm, wbase[-k], Xp));                 // head: rows >= a+1 of the q-tile
+        o = max(o, (int)lookup_cand<Q>(sm, rw2, Xtail));                    // tail: columns <= b-2 of the q-tile
+        oldx = o;
+        // step a6, vertical: the column word now starts at row a
+        const uint32_t xn = (a == Q - 1) ? ((uint32_t)v << C::SH)
+                                         : ((Xp & C::IDXMASK) | ((uint32_t)(v - outv) << (a & 31)) | ((uint32_t)v << C::SH));
+        if (in) Xp = xn;
+        if (a == 0) sm.Xst[A * C::TP + col] = xn;
+        outv = v;
+    }
+}
+
+template <int Q>
+__device__ void closure_offdiag(const Smem<Q> &sm, unsigned long long *tr = nullptr)
+{
+    long long tP = 0, tC = 0;
+    using C = Cfg<Q>;
+    constexpr int NW = C::NTHR / 32;
+    constexpr int QPW = 32 / Q;                 // q-tiles per warp in the C phase
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int grp = lane / Q, b = lane % Q;
+    for (int u = 0; u < 15; ++u) {
+        const int Amax = min(7, 14 - u), Amin = max(0, 7 - u), cnt = Amax - Amin + 1;
+        const long long c0 = clock64();
+        if (u > 0) {
+            for (int t = warp; t < cnt; t += NW) {
+                const int A = Amax - t, B = u - (7 - A);
+                qtile_products<Q>(sm, A, B, A + 1, 8, 8, 8 + B, lane);
+            }
+            __syncthreads();
+        }
+        const long long c1 = clock64();
+        tP += c1 - c0;
+        if (warp * QPW < cnt) {
+            const int t = min(warp * QPW + grp, cnt - 1);
+            const int A = Amax - t, B = u - (7 - A);
+            qtile_closure_fast<Q>(sm, A, B, lane, b);
+        }
+        __syncthreads();
+        tC += clock64() - c1;
+    }
+    if (tr && threadIdx.x == 0) tr[7] = ((unsigned long long)tP << 32) | (unsigned long long)(tC & 0xffffffffll);
+}
+
+// Diagonal super-tile (I == J): only q-tiles with B >= A exist; macro-step u = B - A.  The words a
+// q-tile produces are mirrored into both halves of the word arrays, because here the "static" words
+// of (I,I) / (J,J) are the super-tile's own.
 template <int Q>
 __device__ void closure_diag(const Smem<Q> &sm)
 {
     using C = Cfg<Q>;
-    constexpr int T = C::T;
-    const int tid = threadIdx.x;
-    const int jj = tid >> 2, part = tid & 3;
-    const int gj = jj / Q, pj = jj % Q;
-    const int x = jj + 1;
-    for (int s = 0; s < T; ++s) {
-        const int a = jj - s;
-        const bool active = (a >= 0);
-        uint32_t best = 0;
-        int ga = 0, pa = 0;
-        if (active) {
-            ga = a / Q; pa = a % Q;
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const int g = part + 4 * e;
-                const bool ok = (g >= ga) && (g <= gj) && !(g == ga && pa == Q - 1) && !(g == gj && pj == 0);
-                if (ok) {
-                    const uint32_t W = (g < gj) ? sm.Wst[(8 + g) * C::TP + a] : sm.Wp[a];
-                    const uint32_t X = (g > ga) ? sm.Xst[g * C::TP + jj] : sm.Xp[jj];
-                    const uint32_t S = W + X;
-                    const uint32_t rv = lookup<Q>(sm.tbl, S & C::IDXMASK);
-                    best = max(best, (S >> C::SH) + rv);
-                }
-            }
+    constexpr int NW = C::NTHR / 32;
+    constexpr int QPW = 32 / Q;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int grp = lane / Q, b = lane % Q;
+    for (int u = 0; u < 8; ++u) {
+        const int cnt = 8 - u;
+        if (u >= 2) {
+            for (int t = warp; t < cnt; t += NW) qtile_products<Q>(sm, t, t + u, t + 1, t + u, 0, 0, lane);
+            __syncthreads();
         }
-        best = max(best, __shfl_xor_sync(0xffffffffu, best, 1));
-        best = max(best, __shfl_xor_sync(0xffffffffu, best, 2));
-        if (active && part == 0) {
-            int16_t *vrow = sm.val + a * C::VP;
-            int v = 0;
-            if (s >= 2) {
-                const int dg = vrow[C::VP + x - 1] + rna4r_pair(sm.codeR[a], sm.codeC[jj]);
-                v = max(dg, (int)best);
-            }
-            vrow[x] = (int16_t)v;
-            const int left = vrow[x - 1], below = vrow[C::VP + x];
-            const uint32_t wp = (pj == 0) ? ((uint32_t)v << C::SH)
-                                          : (sm.Wp[a] | ((uint32_t)(v - left) << (C::HB + pj - 1)));
-            sm.Wp[a] = wp;
-            if (pj == Q - 1) sm.Wst[(8 + gj) * C::TP + a] = wp;
-            const uint32_t xp = (pa == Q - 1) ? ((uint32_t)v << C::SH)
-                                              : ((sm.Xp[jj] & C::IDXMASK) | ((uint32_t)(v - below) << pa) | ((uint32_t)v << C::SH));
-            sm.Xp[jj] = xp;
-            if (pa == 0) sm.Xst[ga * C::TP + jj] = xp;
+        if (warp * QPW < cnt) {
+            const int t = warp * QPW + grp;
+            const bool have = (grp < QPW) && (t < cnt);
+            const int A = have ? t : 0, B = A + u;
+            if (u == 0) qtile_closure<Q, true>(sm, have, A, B, A, 8 + B, true, lane, b);
+            else qtile_closure<Q, false>(sm, have, A, B, A, 8 + B, true, lane, b);
         }
         __syncthreads();
     }
@@ -498,6 +643,8 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
     const int nt = si.nt;
     const int dp = J - I;
     const int sidx = si.sbase + tri_index(nt, I, J);
+    unsigned long long *tr = (p.trace && sidx < p.trace_tiles) ? p.trace + (size_t)sidx * 8 : nullptr;
+    if (tr && tid == 0) { tr[0] = global_timer_ns(); tr[6] = ((unsigned long long)I << 32) | (unsigned)J; }
 
     // codes of the rows r = I*T + a (base S[r]) and of the columns c = J*T + jj (base S[c-1])
     if (tid < T) {
@@ -510,7 +657,6 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         // diagonal super-tile: everything starts from zero
         for (int e = tid; e < (T + 1) * C::VP / 2; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.val)[e] = 0;
         for (int e = tid; e < 16 * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
-        if (tid < T) { sm.Wp[tid] = 0; sm.Xp[tid] = 0; }
         __syncthreads();
         closure_diag<Q>(sm);
     } else {
@@ -525,6 +671,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             wait_flag_ge(p.done + s_ii, 1);
             wait_flag_ge(p.done + s_jj, 1);
             if (S > 0) wait_flag_ge(p.accstage + sidx, S);
+            if (tr) tr[1] = global_timer_ns();
         }
         __syncthreads();
         // static words: row words of (I,I) -> Wst[0..7], column words of (J,J) -> Xst[8..15]
@@ -564,6 +711,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             }
         }
         __syncthreads();
+        if (tr && tid == 0) tr[2] = global_timer_ns();
         // late products: the middle blocks whose panels were only finished on the previous step
         if (dp >= 2) {
             const int jj = tid % T, rb = tid / T;
@@ -592,8 +740,10 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             }
             __syncthreads();
         }
-        closure_offdiag<Q>(sm);
+        if (tr && tid == 0) tr[3] = global_timer_ns();
+        closure_offdiag<Q>(sm, tr);
     }
+    if (tr && tid == 0) tr[4] = global_timer_ns();
 
     // ---- publish: row panel, column panel, edges (step a6 output), optional table block, score ----
     {
@@ -627,7 +777,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
         __threadfence();
         __syncthreads();
-        if (tid == 0) st_release_gpu(p.done + sidx, 1);
+        if (tid == 0) { st_release_gpu(p.done + sidx, 1); if (tr) tr[5] = global_timer_ns(); }
     }
 }
 
@@ -740,6 +890,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     p.acc = (int16_t *)(base + w.off_acc);
     p.tbl = C::NIBBLE ? ctx->Rc4 : ctx->Rc;
     p.scores = scores; p.table_out = table_out; p.table_dtype = table_dtype;
+    p.trace = ctx->trace; p.trace_tiles = ctx->trace_tiles;
 
     static bool attr_set = false;
     if (!attr_set) {
@@ -763,7 +914,9 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
         encode_kernel<Q><<<grid, 256, 0, st>>>(p); ++launches;
     }
     size_t want = h.tasks;
-    int blocks = ctx->sm_count * ctx->tiled_blocks_per_sm;
+    int per_sm = ctx->tiled_blocks_per_sm;
+    if (const char *e = getenv("RNA4R_BLOCKS_PER_SM")) { const int v = atoi(e); if (v >= 1 && v < per_sm) per_sm = v; }   // tuning knob
+    int blocks = ctx->sm_count * per_sm;
     if ((size_t)blocks > want) blocks = (int)want;
     if (blocks < 1) blocks = 1;
     if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
