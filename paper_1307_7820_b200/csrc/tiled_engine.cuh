@@ -33,6 +33,10 @@
 
 namespace tiled {
 
+#ifndef RNA4R_ROLES
+#define RNA4R_ROLES 2
+#endif
+
 template <int Q>
 struct Cfg {
     static constexpr int T = 8 * Q;            // cells per super-tile side
@@ -41,14 +45,37 @@ struct Cfg {
     static constexpr uint32_t IDXMASK = (1u << SH) - 1u;
     static constexpr bool NIBBLE = (SH > 16);  // q = 10: nibble-packed table (128 KB)
     static constexpr int TBL_BYTES = NIBBLE ? (1 << SH) / 2 : (1 << SH);
+    // q <= 8: the byte table sits at a shared-memory address aligned to its size, so that the gather
+    // address is (S & IDXMASK) | base -- one LOP3 -- instead of mask + add
+    static constexpr bool TBL_ALIGNED = (Q <= 8);
+    static constexpr int TBL_ALIGN = TBL_ALIGNED ? (TBL_BYTES < 16 ? 16 : TBL_BYTES) : 16;
     static constexpr int NTHR = 4 * T;         // threads per CTA
     static constexpr int RPT = 2 * Q;          // rows per thread in the product phase
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
-    static constexpr int VP = T + 2;           // pitch of the value array (int16)
+    static constexpr int VP = T + 1;           // pitch of the value array (int16): a wavefront step is conflict-free
     static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
     static constexpr int REC_BYTES = 2 * PANEL_WORDS * 4 + 2 * T * 2;   // PH, PV, top row, right column
-    static constexpr size_t SMEM_BYTES =
-        (size_t)((TBL_BYTES + 15) / 16 * 16) + 2 * 16 * TP * 4 + (size_t)(T + 1) * VP * 2 + 2 * 2 * PANEL_WORDS * 4 + 2 * T + 64 + (size_t)(Q + 1) * VP * 2;
+    // closure wavefront: R lanes ("roles") share one column, CPW columns per warp
+    static constexpr int R = RNA4R_ROLES;
+    static constexpr int CPW = 32 / R;
+    static constexpr int NCW = (T + CPW - 1) / CPW;      // wavefront warps (<= NTHR/32)
+    static constexpr int WROWS = 16 + R + 1;             // word-array rows: 16 groups + zero guard rows
+    static constexpr int ESLOTS = T + 2;                 // hand-off slots per warp boundary
+    // shared-memory layout: [E | Wst | Xst | pad | tbl (aligned) | val | stg | codeR | codeC | misc]
+    static constexpr int E_BYTES = 2 * (NCW > 1 ? NCW - 1 : 1) * ESLOTS * 8;
+    static constexpr int W_BYTES = WROWS * TP * 4;
+    static constexpr int PRE_BYTES = (E_BYTES + 2 * W_BYTES + 15) / 16 * 16;
+    static constexpr int VAL_BYTES = (((T + 1) * VP + 1) * 2 + 15) / 16 * 16;
+    static constexpr int STG_BYTES = 2 * 2 * PANEL_WORDS * 4;
+    static constexpr int POST_BYTES = VAL_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64;
+    static_assert(NCW * 32 <= NTHR || T < 32, "wavefront warps must fit the CTA");
+    // dynamic shared memory needed when the dynamic window starts at shared address `base`
+    static constexpr size_t smem_bytes_for(size_t base)
+    {
+        const size_t tbl_at = (base + PRE_BYTES + TBL_ALIGN - 1) / TBL_ALIGN * TBL_ALIGN;
+        return tbl_at - base + (size_t)((TBL_BYTES + 15) / 16 * 16) + POST_BYTES;
+    }
+    static constexpr size_t SMEM_BYTES = smem_bytes_for(0) > smem_bytes_for(1024) ? smem_bytes_for(0) : smem_bytes_for(1024);
 };
 
 struct SeqInfo {
@@ -195,39 +222,60 @@ __global__ void encode_kernel(Params p)
 // ------------------------------------------------------------------------------------------------
 // fill kernel
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
 template <int Q>
 struct Smem {
     using C = Cfg<Q>;
+    uint2 *E;            // [2][NCW-1][ESLOTS] tagged hand-off slots between wavefront warps
+    uint32_t *Wst;       // [WROWS][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own), then zero rows
+    uint32_t *Xst;       // [WROWS][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static), then zero rows
     uint8_t *tbl;        // compact table Rc
-    uint32_t *Wst;       // [16][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own)
-    uint32_t *Xst;       // [16][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static)
+    uint32_t tbl_sa;     // its shared-space address (aligned to TBL_ALIGN)
     int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
     uint32_t *stg;       // [2][2][PANEL_WORDS] product operands, double buffered: [buf][0]=PH, [buf][1]=PV
     int8_t *codeR;       // [T] codes of the rows
     int8_t *codeC;       // [T] codes of the columns
     int *misc;           // [16]
+    bool ok;             // the layout fits the dynamic shared memory of this launch
     __device__ explicit Smem(uint8_t *base)
     {
         uint8_t *p = base;
-        tbl = p; p += (C::TBL_BYTES + 15) / 16 * 16;
-        Wst = (uint32_t *)p; p += 16 * C::TP * 4;
-        Xst = (uint32_t *)p; p += 16 * C::TP * 4;
-        stg = (uint32_t *)p; p += 2 * 2 * C::PANEL_WORDS * 4;
-        val = (int16_t *)p; p += (C::T + 1) * C::VP * 2;
+        E = (uint2 *)p; p += C::E_BYTES;
+        Wst = (uint32_t *)p; p += C::W_BYTES;
+        Xst = (uint32_t *)p; p += C::W_BYTES;
+        const uint32_t sa0 = smem_addr(base);
+        const uint32_t tsa = (sa0 + C::PRE_BYTES + C::TBL_ALIGN - 1) / C::TBL_ALIGN * C::TBL_ALIGN;
+        p = base + (tsa - sa0);
+        tbl = p; tbl_sa = tsa; p += (C::TBL_BYTES + 15) / 16 * 16;
+        val = (int16_t *)p; p += C::VAL_BYTES;
+        stg = (uint32_t *)p; p += C::STG_BYTES;
         codeR = (int8_t *)p; p += C::T;
         codeC = (int8_t *)p; p += C::T;
-        misc = (int *)p;
+        p = base + ((p - base) + 15) / 16 * 16;
+        misc = (int *)p; p += 64;
+        uint32_t dyn;
+        asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+        ok = (uint32_t)(p - base) <= dyn;
     }
 };
 
+// One table gather (the unit of work of this path): rv = Rc[S & IDXMASK].
 template <int Q>
-__device__ __forceinline__ uint32_t lookup(const uint8_t *tbl, uint32_t idx)
+__device__ __forceinline__ uint32_t tbl_gather(const Smem<Q> &sm, uint32_t S)
 {
-    if constexpr (Cfg<Q>::NIBBLE) {
-        const uint32_t w = reinterpret_cast<const uint32_t *>(tbl)[idx >> 3];
+    using C = Cfg<Q>;
+    if constexpr (C::NIBBLE) {
+        const uint32_t idx = S & C::IDXMASK;
+        const uint32_t w = reinterpret_cast<const uint32_t *>(sm.tbl)[idx >> 3];
         return (w >> ((idx & 7u) * 4u)) & 15u;
+    } else if constexpr (C::TBL_ALIGNED) {
+        uint32_t rv;
+        const uint32_t a = (S & C::IDXMASK) | sm.tbl_sa;          // one LOP3: the table is aligned to its size
+        asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"(a));
+        return rv;
     } else {
-        return tbl[idx];
+        return sm.tbl[S & C::IDXMASK];
     }
 }
 
@@ -295,7 +343,7 @@ __device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, u
 #pragma unroll
         for (int rr = 0; rr < C::RPT; ++rr) {
             const uint32_t S = w[rr] + X;
-            const uint32_t rv = lookup<Q>(sm.tbl, S & C::IDXMASK);
+            const uint32_t rv = tbl_gather<Q>(sm, S);
             const uint32_t cand = S + (rv << C::SH);
             acc[rr] = max(acc[rr], cand);
         }
@@ -372,264 +420,165 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA)
+// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA): a continuous skewed wavefront
 //
-// The super-tile is 8 x 8 q-tiles of Q x Q cells; q-tile (A,B) = rows A*Q.., columns B*Q...  q-tiles
-// with equal u = (7-A)+B are independent and are done together (a "macro-step"), in two phases:
-//   P  (all warps, no dependency): every cell of the q-tile takes the maximum over the FULL groups
-//      that lie inside the super-tile's own blocks -- groups x in (A,7] of block I (row words of
-//      (I,I), column words of the q-tiles below, already final) and groups 8..8+B-1 of block J (row
-//      words of the q-tiles to the left, column words of (J,J)).
-//   C  (one lane per column of the q-tile, Q lanes per q-tile): the 2Q-1 anti-diagonal steps
-//       inside the q-tile.  A lane walks its column bottom-up; the running row word
-//      and the neighbour values travel lane to lane by shuffles, the running column word stays in a
-//      register, so a cell-step costs no CTA barrier.  The paper's two residual loops
-//       are the two MASKED lookups: head = (row word of (I,I), running column
-//      word), tail = (running row word, column word of (J,J)).
+// Local coordinates: rows a = 0..T-1 (a = T-1 is the bottom row), columns c = 0..T-1.  Lane <-> column:
+// the lane that owns column c walks it bottom-up, one cell per step, one row below its left
+// neighbour: at step k it is on row a = T-1-k+c, so all cells of one anti-diagonal
+// are computed in the same step and the whole tile takes 2T-1 steps, with no barrier between them.
+// CPW = 32/R columns per warp; the R lanes ("roles") of a column hold identical wavefront state and
+// split the table lookups of the step.  Neighbouring warps are coupled by tagged hand-off slots in
+// shared memory (value + row word of the warp's last two columns), polled by the consumer.
+//
+// Critical-path split.  Of all candidates of cell (a,c) only two depend on the previous step:
+//   left  = v(a,c-1)  (tail split t = c-1: M(r,c-1) + M(c-1,c), M(c-1,c) = 0)   -- one shuffle
+//   below = v(a+1,c)  (head split t = r+1: M(r,r+1) + M(r+1,c), M(r,r+1) = 0)   -- own register.
+// Everything else of cell (a-1,c) -- the bulk maximum, b + D(i+1,j-1) and every
+// lookup over rows >= a+1 and columns <= c-2 -- is computed during step k ("OLDX") and only enters
+// v(a-1,c) at step k+1.  So the dependent chain of a step is  shuffle -> max.
+//
+// Lookups of one step, target cell (a-1,c).  With the word arrays indexed by z = 0..15 (z < 8: group
+// z of block I, z >= 8: group z-8 of block J) the groups to look up are one contiguous range
+// z = zL..zR,  zL = floor((a+1)/Q),  zR = 8 + floor((c-2)/Q):
+//   z = zL  head special: the running column word Xp (rows >= a+1 of the lane's own column) with the
+//           row word of (I,I)                                 -- the paper's head residual loop
+//   z = zR  tail special: the row word of row a-1 through column c-2 (from lane c-2, by shuffle) with
+//           the column word of (J,J)                          -- the paper's tail residual loop
+//   zL < z < zR  interior: both words complete, read from shared memory (full groups)
+// (PAPER.md:145-155 residual loops as masked lookups: DESIGN.md 4.3).  Words that are not complete yet
+// are zero (the arrays are cleared per tile), and a zero word only yields a valid lower bound, so the
+// walk over the interior may overshoot without harm; its trip count is warp-uniform.
+// DIAG (I == J): row and column words are both the tile's own; only z < 8 is used (zR = floor((c-2)/Q)),
+// plus the merged lookup (row word through c-2, Xp) when zL == zR; cells with c-a <= 1 are 0.
 // ------------------------------------------------------------------------------------------------
+constexpr uint32_t E_TAG = 0x5a5a0000u;
+
+__device__ __forceinline__ uint2 lds_volatile_u2(const uint2 *p)
+{
+    uint2 r;
+    asm volatile("ld.volatile.shared.v2.u32 {%0, %1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(smem_addr(p)) : "memory");
+    return r;
+}
+__device__ __forceinline__ void sts_volatile_u2(uint2 *p, uint32_t x, uint32_t y)
+{
+    asm volatile("st.volatile.shared.v2.u32 [%0], {%1, %2};" ::"r"(smem_addr(p)), "r"(x), "r"(y) : "memory");
+}
+
 template <int Q>
-__device__ __forceinline__ uint32_t lookup_cand(const Smem<Q> &sm, uint32_t W, uint32_t X)
+__device__ __forceinline__ uint32_t lookup_tagged(const Smem<Q> &sm, uint32_t W, uint32_t X)
 {
     const uint32_t S = W + X;
-    return (S >> Cfg<Q>::SH) + lookup<Q>(sm.tbl, S & Cfg<Q>::IDXMASK);
+    return S + (tbl_gather<Q>(sm, S) << Cfg<Q>::SH);      // (value << SH) | harmless low bits
 }
 
-// P phase for q-tile (A,B), executed by one warp.  Word-array indices [x0,x1) and [y0,y1).
-template <int Q>
-__device__ __forceinline__ void qtile_products(const Smem<Q> &sm, int A, int B, int x0, int x1, int y0, int y1, int lane)
+template <int Q, bool DIAG>
+__device__ __forceinline__ void wave_closure(const Smem<Q> &sm, int cw, int lane)
 {
     using C = Cfg<Q>;
-    constexpr int CPL = (Q * Q + 31) / 32;     // cells per lane
-    int row[CPL], col[CPL];
-    uint32_t best[CPL];
-#pragma unroll
-    for (int c = 0; c < CPL; ++c) {
-        int e = lane + 32 * c;
-        if (e >= Q * Q) e = Q * Q - 1;           // surplus lanes redo the last cell (same value, benign)
-        row[c] = A * Q + e / Q;
-        col[c] = B * Q + e % Q;
-        best[c] = 0;
-    }
-#pragma unroll 2
-    for (int x = x0; x < x1; ++x) {
-#pragma unroll
-        for (int c = 0; c < CPL; ++c)
-            best[c] = max(best[c], lookup_cand<Q>(sm, sm.Wst[x * C::TP + row[c]], sm.Xst[x * C::TP + col[c]]));
-    }
-#pragma unroll 2
-    for (int y = y0; y < y1; ++y) {
-#pragma unroll
-        for (int c = 0; c < CPL; ++c)
-            best[c] = max(best[c], lookup_cand<Q>(sm, sm.Wst[y * C::TP + row[c]], sm.Xst[y * C::TP + col[c]]));
-    }
-#pragma unroll
-    for (int c = 0; c < CPL; ++c) {
-        int16_t *cell = sm.val + row[c] * C::VP + col[c] + 1;
-        const int cur = *cell;
-        if ((int)best[c] > cur && lane + 32 * c < Q * Q) *cell = (int16_t)best[c];
-    }
-}
+    constexpr int T = C::T, TP = C::TP, VP = C::VP, SH = C::SH, HB = C::HB, R = C::R, CPW = C::CPW, NCW = C::NCW;
+    constexpr uint32_t FULL = 0xffffffffu;
+    constexpr int OFFQ = 64 * Q;                         // keeps the operand of the constant divisions positive
+    const int j = lane % CPW, rho = lane / CPW;
+    const int c = cw * CPW + j;                          // my column (>= T: idle lane, never stores)
+    const bool colok = c < T;
+    const int b = c % Q, B = c / Q;
+    const int zR = (DIAG ? 0 : 8) + (c >= 2 ? (c - 2) / Q : 0);
+    const uint32_t w2keep = (c >= 2) ? FULL : 0u;
+    const int want = 3 - (int)sm.codeC[colok ? c : 0];   // row code that pairs with my column (code 4 -> never)
+    const int B0c = sm.val[T * VP + c + 1];              // bottom edge M((I+1)T, c)
+    const uint32_t XR = DIAG ? 0u : sm.Xst[zR * TP + c]; // static column word of (J,J) for the tail special
+    const int shb = HB + (b > 0 ? b - 1 : 0);            // position of my horizontal difference bit
+    uint2 *E1 = sm.E + (size_t)(2 * cw) * C::ESLOTS, *E2 = E1 + C::ESLOTS;             // slots I produce
+    const uint2 *P1 = sm.E + (size_t)(2 * (cw > 0 ? cw - 1 : 0)) * C::ESLOTS, *P2 = P1 + C::ESLOTS;   // slots I consume
+    const int k0 = cw * CPW - 1;                         // pre-step of my first column
+    const int kstart = DIAG ? max(k0, T) : k0;
+    const int kend = min(T - 1 + (cw + 1) * CPW - 1, 2 * T - 2);
+    const bool r0 = (rho == 0);
 
-// C phase for q-tile (A,B): lane b (0..Q-1 of its group) owns column b and walks it bottom-up, one
-// cell per step; lane b works one row below lane b-1, so row data flows lane to lane by shuffles.
-// `have` = this lane group has a q-tile.  hg / tg: word-array rows with the head row words / tail
-// column words.
-//
-// Critical-path split.  Of all candidates of cell (a,b) only two depend on the previous step:
-//   left  = v(a,b-1)  (tail split t = c-1: M(r,c-1) + M(c-1,c), M(c-1,c) = 0)
-//   below = v(a+1,b)  (head split t = r+1: M(r,r+1) + M(r+1,c), M(r,r+1) = 0).
-// Everything else -- the bulk maximum, b + D(i+1,j-1), the head lookup over rows >= a+2 and the tail
-// lookup over columns <= b-2 -- is known one step earlier and is folded into OLDX during the previous
-// step.  So the dependent chain of a step is  shuffle -> max -> max.
-//
-// DIAGQ: the q-tile lies on the main diagonal (A == B of a diagonal super-tile): cells with b-a <= 1
-// are 0, rows start at b == a, and head and tail merge into one lookup with both words running.
-template <int Q, bool DIAGQ>
-__device__ __forceinline__ void qtile_closure(const Smem<Q> &sm, bool have, int A, int B, int hg, int tg, bool mirror,
-                                              int lane, int b)
-{
-    using C = Cfg<Q>;
-    const int row0 = A * Q, col = B * Q + b, x = col + 1;
-    const int src1 = (b > 0) ? lane - 1 : lane, src2 = (b > 1) ? lane - 2 : lane;
-    uint32_t Xtail = 0, pm = 0;
-    if (have) {
-        Xtail = sm.Xst[tg * C::TP + col];
-        const int cc = sm.codeC[col];
-#pragma unroll
-        for (int a = 0; a < Q; ++a) pm |= (uint32_t)rna4r_pair(sm.codeR[row0 + a], cc) << a;
-    }
-    uint32_t Xp = 0;        // running column word: rows below the current cell
-    uint32_t outword = 0;   // row word of my last cell's row, my cell included
-    int outv = 0;           // my last value
-    int oldx = 0;           // OLDX of my next cell
-#pragma unroll
-    for (int k = (DIAGQ ? Q - 1 : -1); k < 2 * Q - 1; ++k) {
-        const int L = __shfl_sync(0xffffffffu, outv, src1);                 // v(a, b-1)
-        const uint32_t rw1 = __shfl_sync(0xffffffffu, outword, src1);       // row a,   columns <= b-1
-        const uint32_t rw2 = __shfl_sync(0xffffffffu, outword, src2);       // row a-1, columns <= b-2
-        const int a = Q - 1 - k + b;
-        if (have && a >= 0 && a <= Q) {
-            const int row = row0 + a;
-            int16_t *vrow = sm.val + row * C::VP;
-            int v;
-            if (a < Q) {
-                v = max(oldx, outv);                                        // OLDX, below
-                if (b > 0) v = max(v, L);                                   // left
-                if (DIAGQ && b - a <= 1) v = 0;
-                vrow[x] = (int16_t)v;
-                // step a6: append the horizontal difference bit to the row word
-                const uint32_t myrow = (b == 0 || (DIAGQ && b == a)) ? ((uint32_t)v << C::SH)
-                                                                      : (rw1 | ((uint32_t)(v - L) << (C::HB + b - 1)));
-                outword = myrow;
-                if (b == Q - 1) {
-                    sm.Wst[(8 + B) * C::TP + row] = myrow;
-                    if (mirror) sm.Wst[B * C::TP + row] = myrow;
-                }
-            } else {
-                v = vrow[x];                                                // the cell below the q-tile
+    int vout = 0, vprev = 0, oldx = 0;
+    uint32_t wout = 0, Xp = 0;
+#pragma unroll 1
+    for (int k = kstart; k <= kend; ++k) {
+        const int a = T - 1 - k + c;
+        const int d = k - (T - 1);                       // c - a, the same for every lane
+        // ---- receive from the left
+        int Lv = __shfl_up_sync(FULL, vout, 1, CPW);                // v(a, c-1)
+        uint32_t Lw = __shfl_up_sync(FULL, wout, 1, CPW);           // row a   through column c-1
+        uint32_t Lw2 = __shfl_up_sync(FULL, wout, 2, CPW);          // row a-1 through column c-2
+        if (cw == 0) {
+            if (j == 0) Lv = sm.val[a * VP];                        // left edge (a = T: the corner)
+            if (j < 2) Lw2 = 0;
+        } else {
+            const int a0 = T - 1 - k + cw * CPW;                    // row of my first column, warp-uniform
+            uint2 e1 = make_uint2(0u, 0u), e2 = make_uint2(0u, 0u);
+            if (!(DIAG && k == T)) {                                // DIAG: step T-1 is not run, its cells are 0
+                if (a0 >= 0)
+                    for (;;) { e1 = lds_volatile_u2(P1 + a0); if (__all_sync(FULL, (e1.x & 0xffff0000u) == E_TAG)) break; }
+                if (a0 >= 1)
+                    for (;;) { e2 = lds_volatile_u2(P2 + a0 - 1); if (__all_sync(FULL, (e2.x & 0xffff0000u) == E_TAG)) break; }
             }
-            if (a >= 1) {                                                   // OLDX of cell (a-1, b)
-                int o = vrow[x - C::VP];                                    // bulk + P-phase maximum
-                const int dgv = (b == 0 || a == Q) ? (int)vrow[x - 1] : L;  // D(i+1,j-1) = v(a, b-1)
-                o = max(o, dgv + (int)((pm >> (a - 1)) & 1u));              // + b(S_i,S_j)
-                if (DIAGQ) {
-                    if (b >= 2) o = max(o, (int)lookup_cand<Q>(sm, rw2, Xp));
-                } else {
-                    if (a <= Q - 2) o = max(o, (int)lookup_cand<Q>(sm, sm.Wst[hg * C::TP + row - 1], Xp));   // head, rows >= a+1
-                    if (b >= 2) o = max(o, (int)lookup_cand<Q>(sm, rw2, Xtail));                             // tail, cols <= b-2
-                }
-                oldx = o;
-            }
-            if (a < Q) {
-                // step a6: append the vertical difference bit to the column word (now rows >= a)
-                Xp = (a == Q - 1) ? ((uint32_t)v << C::SH)
-                                  : ((Xp & C::IDXMASK) | ((uint32_t)(v - outv) << a) | ((uint32_t)v << C::SH));
-                if (a == 0) {
-                    sm.Xst[A * C::TP + col] = Xp;
-                    if (mirror) sm.Xst[(8 + A) * C::TP + col] = Xp;
-                }
-            }
-            outv = v;
+            if (j == 0) { Lv = (int)(e1.x & 0xffffu); Lw = e1.y; Lw2 = e2.y; }
+            if (j == 1) Lw2 = e1.y;
         }
-    }
-}
-
-// Branch-free C phase for the q-tiles of an off-diagonal super-tile (the hot variant of
-// qtile_closure<Q,false>; same recurrence, same fresh/old split).  Every lane group runs a q-tile
-// (surplus groups redo the last one: identical values, benign), every lane runs every step, and
-//   * outside its window (steps b-1 .. b+Q-1) a lane computes don't-care values and stores nothing;
-//   * a lookup whose operand does not exist is fed a zero word, which makes it a valid lower bound:
-//     W = 0 gives M(gq,c) <= M(r,c), X = 0 gives max of the row run <= M(r,c) (Lemma 1 monotonicity);
-//   * all shared-memory addresses are affine in the step index, so the unrolled steps use immediate
-//     offsets (out-of-window loads land in the padded neighbourhood of the arrays and are ignored).
-template <int Q>
-__device__ __forceinline__ void qtile_closure_fast(const Smem<Q> &sm, int A, int B, int lane, int b)
-{
-    using C = Cfg<Q>;
-    const int row0 = A * Q, col = B * Q + b, x = col + 1;
-    const int src1 = (b > 0) ? lane - 1 : lane, src2 = (b > 1) ? lane - 2 : lane;
-    const uint32_t Xtail = sm.Xst[(8 + B) * C::TP + col];
-    uint32_t pm = 0;
-    {
-        const int cc = sm.codeC[col];
+        // ---- the cell (a3 init + a5 fresh splits)
+        int v = max(max(oldx, vprev), Lv);
+        if (a == T) v = B0c;                                        // pre-step: the cell below the tile
+        if (DIAG && d <= 1) v = 0;                                  // D(i,i) = D(i,i-1) = 0
+        const bool live = colok && (unsigned)a < (unsigned)T;
+        if (live && r0) sm.val[a * VP + c + 1] = (int16_t)v;
+        // ---- step a6, horizontal: my row word = neighbour's word | my difference bit
+        const uint32_t wme = (b == 0) ? ((uint32_t)v << SH) : (Lw | ((uint32_t)(v - Lv) << shb));
+        if (live && r0 && b == Q - 1) {
+            sm.Wst[(8 + B) * TP + a] = wme;
+            if (DIAG) sm.Wst[B * TP + a] = wme;
+        }
+        if (cw < NCW - 1 && r0 && colok && (unsigned)a <= (unsigned)T) {
+            if (j == CPW - 1) sts_volatile_u2(E1 + a, E_TAG | (uint32_t)(v & 0xffff), wme);
+            if (j == CPW - 2) sts_volatile_u2(E2 + a, E_TAG, wme);
+        }
+        // ---- OLDX of the next cell (a-1, c)
+        int o = sm.val[(a - 1) * VP + c + 1];                       // bulk maximum
+        if ((int)sm.codeR[a - 1] == want) o = max(o, Lv + 1);       // b(S_i,S_j) + D(i+1,j-1)
+        const int zL = min((int)((unsigned)(a + 1 + OFFQ) / Q) - 64, 7);   // floor((a+1)/Q); 7 when no row of the tile is below
+        const int fl = (int)((unsigned)(d - 3 + OFFQ) / Q) - 64;    // floor((d-3)/Q), warp-uniform
+        // warp-uniform upper bound of the interior count zR-zL-1: floor differences give 8+fl; one more because
+        // zR is one too high for columns 0,1 (no tail group) and zL is clamped on the bottom row
+        const int nint = min(DIAG ? fl : 9 + fl, DIAG ? 6 : 14);
+        const int nit = nint > 0 ? (nint + R - 1) / R : 0;
+        const uint32_t Wh = sm.Wst[zL * TP + a - 1];
+        const uint32_t Xt = DIAG ? sm.Xst[zR * TP + c] : XR;
+        const uint32_t Lw2m = Lw2 & w2keep;
+        uint32_t best;
+        if (R == 1) {
+            best = max(lookup_tagged<Q>(sm, Wh, Xp), lookup_tagged<Q>(sm, Lw2m, Xt));
+        } else {
+            const uint32_t W0 = (rho == 0) ? Wh : (rho == 1 ? Lw2m : 0u);
+            const uint32_t X0 = (rho == 0) ? Xp : (rho == 1 ? Xt : 0u);
+            best = lookup_tagged<Q>(sm, W0, X0);
+        }
+        if (DIAG) best = max(best, lookup_tagged<Q>(sm, (zL == zR) ? Lw2m : 0u, Xp));
+        {
+            const uint32_t *pw = sm.Wst + (zL + 1 + rho) * TP + a - 1;
+            const uint32_t *px = sm.Xst + (zL + 1 + rho) * TP + c;
+            constexpr int NITMAX = ((DIAG ? 6 : 14) + R - 1) / R;
 #pragma unroll
-        for (int a = 0; a < Q; ++a) pm |= (uint32_t)rna4r_pair(sm.codeR[row0 + a], cc) << (a + 1);   // bit a+1 <-> row a
-    }
-    // lane-affine bases: at step k the lane is on row  a = Q-1-k+b
-    int16_t *vbase = sm.val + (row0 + Q - 1 + b) * C::VP + x;           // vbase[-k*VP] = val[row][x]
-    const uint32_t *wbase = sm.Wst + A * C::TP + row0 + Q - 2 + b;      // wbase[-k]    = Wst[A][row-1]
-    uint32_t *wout = sm.Wst + (8 + B) * C::TP + row0 + Q - 1 + b;       // wout[-k]     = Wst[8+B][row]
-    const uint32_t rw2mask = (b >= 2) ? 0xffffffffu : 0u;
-    const bool lastcol = (b == Q - 1), firstcol = (b == 0);
-    const int shb = C::HB + b - 1;                                      // position of my horizontal bit
-    uint32_t Xp = 0, outword = 0;
-    int outv = 0, oldx = 0;
-#pragma unroll
-    for (int k = -1; k < 2 * Q - 1; ++k) {
-        const int L = __shfl_sync(0xffffffffu, outv, src1);                 // v(a, b-1)
-        const uint32_t rw1 = __shfl_sync(0xffffffffu, outword, src1);       // row a,   columns <= b-1
-        const uint32_t rw2 = __shfl_sync(0xffffffffu, outword, src2) & rw2mask;   // row a-1, columns <= b-2
-        const int a = Q - 1 - k + b;
-        const bool in = (unsigned)a < (unsigned)Q;
-        int v = max(max(oldx, outv), L);                                    // OLDX, below, left
-        if (a == Q) v = vbase[-k * C::VP];                                  // pre-step: the cell below the q-tile
-        if (in) vbase[-k * C::VP] = (int16_t)v;
-        // step a6, horizontal: my row word = neighbour's word | my difference bit
-        const uint32_t myrow = firstcol ? ((uint32_t)v << C::SH) : (rw1 | ((uint32_t)(v - L) << shb));
-        outword = myrow;
-        if (in && lastcol) wout[-k] = myrow;
-        // OLDX of the next cell (a-1, b)
-        const int dgv = (firstcol || a == Q) ? (int)vbase[-k * C::VP - 1] : L;      // D(i+1,j-1)
-        int o = max((int)vbase[-(k + 1) * C::VP], dgv + (int)((pm >> (a & 31)) & 1u));
-        o = max(o, (int)lookup_cand<Q>(sm, wbase[-k], Xp));                 // head: rows >= a+1 of the q-tile
-        o = max(o, (int)lookup_cand<Q>(sm, rw2, Xtail));                    // tail: columns <= b-2 of the q-tile
-        oldx = o;
-        // step a6, vertical: the column word now starts at row a
-        const uint32_t xn = (a == Q - 1) ? ((uint32_t)v << C::SH)
-                                         : ((Xp & C::IDXMASK) | ((uint32_t)(v - outv) << (a & 31)) | ((uint32_t)v << C::SH));
-        if (in) Xp = xn;
-        if (a == 0) sm.Xst[A * C::TP + col] = xn;
-        outv = v;
-    }
-}
-
-template <int Q>
-__device__ void closure_offdiag(const Smem<Q> &sm, unsigned long long *tr = nullptr)
-{
-    long long tP = 0, tC = 0;
-    using C = Cfg<Q>;
-    constexpr int NW = C::NTHR / 32;
-    constexpr int QPW = 32 / Q;                 // q-tiles per warp in the C phase
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int grp = lane / Q, b = lane % Q;
-    for (int u = 0; u < 15; ++u) {
-        const int Amax = min(7, 14 - u), Amin = max(0, 7 - u), cnt = Amax - Amin + 1;
-        const long long c0 = clock64();
-        if (u > 0) {
-            for (int t = warp; t < cnt; t += NW) {
-                const int A = Amax - t, B = u - (7 - A);
-                qtile_products<Q>(sm, A, B, A + 1, 8, 8, 8 + B, lane);
+            for (int i = 0; i < NITMAX; ++i) {
+                if (i < nit) best = max(best, lookup_tagged<Q>(sm, pw[i * R * TP], px[i * R * TP]));
             }
-            __syncthreads();
         }
-        const long long c1 = clock64();
-        tP += c1 - c0;
-        if (warp * QPW < cnt) {
-            const int t = min(warp * QPW + grp, cnt - 1);
-            const int A = Amax - t, B = u - (7 - A);
-            qtile_closure_fast<Q>(sm, A, B, lane, b);
+        if (R >= 2) best = max(best, __shfl_xor_sync(FULL, best, CPW));
+        if (R >= 4) best = max(best, __shfl_xor_sync(FULL, best, 2 * CPW));
+        oldx = max(o, (int)(best >> SH));
+        // ---- step a6, vertical: the column word now starts at row a
+        const int am = (int)((unsigned)(a + OFFQ) % Q);
+        if (a >= T) {
+            Xp = 0;                                                 // nothing of my column is known below the tile
+        } else {
+            Xp = (am == Q - 1) ? ((uint32_t)v << SH)
+                               : ((Xp & C::IDXMASK) | ((uint32_t)(v - vprev) << am) | ((uint32_t)v << SH));
+            if (live && r0 && am == 0) sm.Xst[(a / Q) * TP + c] = Xp;
         }
-        __syncthreads();
-        tC += clock64() - c1;
-    }
-    if (tr && threadIdx.x == 0) tr[7] = ((unsigned long long)tP << 32) | (unsigned long long)(tC & 0xffffffffll);
-}
-
-// Diagonal super-tile (I == J): only q-tiles with B >= A exist; macro-step u = B - A.  The words a
-// q-tile produces are mirrored into both halves of the word arrays, because here the "static" words
-// of (I,I) / (J,J) are the super-tile's own.
-template <int Q>
-__device__ void closure_diag(const Smem<Q> &sm)
-{
-    using C = Cfg<Q>;
-    constexpr int NW = C::NTHR / 32;
-    constexpr int QPW = 32 / Q;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int grp = lane / Q, b = lane % Q;
-    for (int u = 0; u < 8; ++u) {
-        const int cnt = 8 - u;
-        if (u >= 2) {
-            for (int t = warp; t < cnt; t += NW) qtile_products<Q>(sm, t, t + u, t + 1, t + u, 0, 0, lane);
-            __syncthreads();
-        }
-        if (warp * QPW < cnt) {
-            const int t = warp * QPW + grp;
-            const bool have = (grp < QPW) && (t < cnt);
-            const int A = have ? t : 0, B = A + u;
-            if (u == 0) qtile_closure<Q, true>(sm, have, A, B, A, 8 + B, true, lane, b);
-            else qtile_closure<Q, false>(sm, have, A, B, A, 8 + B, true, lane, b);
-        }
-        __syncthreads();
+        vprev = v; vout = v; wout = wme;
     }
 }
 
@@ -653,12 +602,16 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         sm.codeC[tid] = (c >= 1) ? p.codes[si.cbase + c - 1] : (int8_t)4;
     }
 
+    const int warp = tid >> 5, lane = tid & 31;
+    // hand-off slots of the wavefront warps: empty
+    for (int e = tid; e < C::E_BYTES / 8; e += C::NTHR) sm.E[e] = make_uint2(0u, 0u);
     if (dp == 0) {
         // diagonal super-tile: everything starts from zero
-        for (int e = tid; e < (T + 1) * C::VP / 2; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.val)[e] = 0;
-        for (int e = tid; e < 16 * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
+        for (int e = tid; e < C::VAL_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.val)[e] = 0;
+        for (int e = tid; e < C::WROWS * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
         __syncthreads();
-        closure_diag<Q>(sm);
+        if (warp < C::NCW) wave_closure<Q, true>(sm, warp, lane);
+        __syncthreads();
     } else {
         const int s_left = si.sbase + tri_index(nt, I, J - 1);
         const int s_below = si.sbase + tri_index(nt, I + 1, J);
@@ -683,6 +636,10 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
                 sm.Wst[g * C::TP + k] = __ldcg(ph + e);
                 sm.Xst[(8 + g) * C::TP + k] = __ldcg(pv + e);
             }
+            // the tile's own words are not known yet: zero (= a valid lower bound); zero guard rows
+            for (int e = tid; e < (C::WROWS - 8) * C::TP; e += C::NTHR) sm.Wst[8 * C::TP + e] = 0;
+            for (int e = tid; e < 8 * C::TP; e += C::NTHR) sm.Xst[e] = 0;
+            for (int e = tid; e < (C::WROWS - 16) * C::TP; e += C::NTHR) sm.Xst[16 * C::TP + e] = 0;
         }
         // bulk maxima gathered by the PROD stages (or zero)
         if (S > 0) {
@@ -741,7 +698,8 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             __syncthreads();
         }
         if (tr && tid == 0) tr[3] = global_timer_ns();
-        closure_offdiag<Q>(sm, tr);
+        if (warp < C::NCW) wave_closure<Q, false>(sm, warp, lane);
+        __syncthreads();
     }
     if (tr && tid == 0) tr[4] = global_timer_ns();
 
@@ -788,6 +746,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR) fill_kernel(Params p)
     extern __shared__ __align__(16) uint8_t smem_raw[];
     Smem<Q> sm(smem_raw);
     const int tid = threadIdx.x;
+    if (!sm.ok) __trap();                      // the host sized the launch for another shared-memory base: fail loudly
     // table R (reachable quadrant) -> shared memory, once per CTA
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(p.tbl);
