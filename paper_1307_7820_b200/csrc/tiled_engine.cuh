@@ -33,10 +33,6 @@
 
 namespace tiled {
 
-#ifndef RNA4R_ROLES
-#define RNA4R_ROLES 2
-#endif
-
 template <int Q>
 struct Cfg {
     static constexpr int T = 8 * Q;            // cells per super-tile side
@@ -49,26 +45,25 @@ struct Cfg {
     // address is (S & IDXMASK) | base -- one LOP3 -- instead of mask + add
     static constexpr bool TBL_ALIGNED = (Q <= 8);
     static constexpr int TBL_ALIGN = TBL_ALIGNED ? (TBL_BYTES < 16 ? 16 : TBL_BYTES) : 16;
-    static constexpr int NTHR = 4 * T;         // threads per CTA
+    static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
+    static constexpr int NTHR = PTHR > 256 ? PTHR : 256;   // threads per CTA: at least the 8 closure warps
     static constexpr int RPT = 2 * Q;          // rows per thread in the product phase
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
     static constexpr int VP = T + 1;           // pitch of the value array (int16): a wavefront step is conflict-free
     static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
     static constexpr int REC_BYTES = 2 * PANEL_WORDS * 4 + 2 * T * 2;   // PH, PV, top row, right column
-    // closure wavefront: R lanes ("roles") share one column, CPW columns per warp
-    static constexpr int R = RNA4R_ROLES;
-    static constexpr int CPW = 32 / R;
-    static constexpr int NCW = (T + CPW - 1) / CPW;      // wavefront warps (<= NTHR/32)
-    static constexpr int WROWS = 16 + R + 1;             // word-array rows: 16 groups + zero guard rows
-    static constexpr int ESLOTS = T + 2;                 // hand-off slots per warp boundary
-    // shared-memory layout: [E | Wst | Xst | pad | tbl (aligned) | val | stg | codeR | codeC | misc]
-    static constexpr int E_BYTES = 2 * (NCW > 1 ? NCW - 1 : 1) * ESLOTS * 8;
+    static constexpr int WROWS = 16;           // word-array rows: 8 groups of block I, 8 of block J
+    // shared-memory layout: [guard | Wst | Xst | pad | tbl (aligned) | val (guard rows around) | stg | codeR | codeC | misc | mbar]
+    // The unrolled closure steps address val and Wst with immediate offsets; lanes outside their window
+    // read up to Q rows beyond either end of the arrays (values ignored): the guards keep those reads inside.
+    static constexpr int W_GUARD = 64;         // bytes before Wst
     static constexpr int W_BYTES = WROWS * TP * 4;
-    static constexpr int PRE_BYTES = (E_BYTES + 2 * W_BYTES + 15) / 16 * 16;
-    static constexpr int VAL_BYTES = (((T + 1) * VP + 1) * 2 + 15) / 16 * 16;
+    static constexpr int PRE_BYTES = (W_GUARD + 2 * W_BYTES + 15) / 16 * 16;
+    static constexpr int VAL_ROWS = T + 1 + 2 * Q;   // Q guard rows, rows 0..T, Q guard rows
+    static constexpr int VAL_BYTES = ((VAL_ROWS * VP + 2) * 2 + 15) / 16 * 16;
     static constexpr int STG_BYTES = 2 * 2 * PANEL_WORDS * 4;
-    static constexpr int POST_BYTES = VAL_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64;
-    static_assert(NCW * 32 <= NTHR || T < 32, "wavefront warps must fit the CTA");
+    static constexpr int MBAR_BYTES = 64 * 8;  // one mbarrier per q-tile: warp B -> warp B+1 hand-off
+    static constexpr int POST_BYTES = VAL_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
     // dynamic shared memory needed when the dynamic window starts at shared address `base`
     static constexpr size_t smem_bytes_for(size_t base)
     {
@@ -227,33 +222,35 @@ __device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)
 template <int Q>
 struct Smem {
     using C = Cfg<Q>;
-    uint2 *E;            // [2][NCW-1][ESLOTS] tagged hand-off slots between wavefront warps
-    uint32_t *Wst;       // [WROWS][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own), then zero rows
-    uint32_t *Xst;       // [WROWS][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static), then zero rows
+    uint32_t *Wst;       // [WROWS][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own)
+    uint32_t *Xst;       // [WROWS][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static)
     uint8_t *tbl;        // compact table Rc
     uint32_t tbl_sa;     // its shared-space address (aligned to TBL_ALIGN)
+    int16_t *valraw;     // start of the value array including its guard rows
     int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
     uint32_t *stg;       // [2][2][PANEL_WORDS] product operands, double buffered: [buf][0]=PH, [buf][1]=PV
     int8_t *codeR;       // [T] codes of the rows
     int8_t *codeC;       // [T] codes of the columns
     int *misc;           // [16]
+    uint64_t *mbar;      // [8][8] mbarrier of q-tile (A,B) at mbar[B*8+A]: completes once per closure
     bool ok;             // the layout fits the dynamic shared memory of this launch
     __device__ explicit Smem(uint8_t *base)
     {
         uint8_t *p = base;
-        E = (uint2 *)p; p += C::E_BYTES;
+        p += C::W_GUARD;
         Wst = (uint32_t *)p; p += C::W_BYTES;
         Xst = (uint32_t *)p; p += C::W_BYTES;
         const uint32_t sa0 = smem_addr(base);
         const uint32_t tsa = (sa0 + C::PRE_BYTES + C::TBL_ALIGN - 1) / C::TBL_ALIGN * C::TBL_ALIGN;
         p = base + (tsa - sa0);
         tbl = p; tbl_sa = tsa; p += (C::TBL_BYTES + 15) / 16 * 16;
-        val = (int16_t *)p; p += C::VAL_BYTES;
+        valraw = (int16_t *)p; val = valraw + Q * C::VP; p += C::VAL_BYTES;     // val[0] = row 0; Q guard rows on either side
         stg = (uint32_t *)p; p += C::STG_BYTES;
         codeR = (int8_t *)p; p += C::T;
         codeC = (int8_t *)p; p += C::T;
         p = base + ((p - base) + 15) / 16 * 16;
         misc = (int *)p; p += 64;
+        mbar = (uint64_t *)p; p += C::MBAR_BYTES;
         uint32_t dyn;
         asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
         ok = (uint32_t)(p - base) <= dyn;
@@ -306,7 +303,7 @@ __device__ __forceinline__ void load_operands_async(const Params &p, const Smem<
     uint32_t *dst = sm.stg + (size_t)buf * 2 * C::PANEL_WORDS;
     if (tid < CH) {
         cp_async16(dst + tid * 4, rec_ptr<Q>(p, sidx_ik) + (size_t)tid * 16);                               // PH of (I,K)
-    } else {
+    } else if (tid < 2 * CH) {
         const int c = tid - CH;
         cp_async16(dst + C::PANEL_WORDS + c * 4, rec_ptr<Q>(p, sidx_kj) + (size_t)C::PANEL_WORDS * 4 + (size_t)c * 16);   // PV of (K,J)
     }
@@ -362,7 +359,8 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
     const int hi = dp - 2 - s * p.delta;
     const int lo = max(hi - p.delta + 1, (dp + 1) / 2);
     const int sidx = si.sbase + tri_index(nt, I, J);
-    const int jj = tid % C::T, rb = tid / C::T;
+    const bool pact = tid < C::PTHR;             // threads beyond 4T only help with barriers (q < 8)
+    const int jj = tid % C::T, rb = pact ? tid / C::T : 0;
     uint32_t acc[C::RPT];
 #pragma unroll
     for (int rr = 0; rr < C::RPT; ++rr) acc[rr] = 0;
@@ -396,7 +394,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
         const bool more = issue_next();
         if (more) cp_async_wait<1>(); else cp_async_wait<0>();
         __syncthreads();
-        product_accumulate<Q>(sm, computed & 1, acc, jj, rb);
+        if (pact) product_accumulate<Q>(sm, computed & 1, acc, jj, rb);
         ++computed;
         __syncthreads();     // the buffer may be refilled by the next issue
     }
@@ -405,181 +403,217 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
     if (s != S - 1) {
         if (tid == 0) wait_flag_ge(p.accstage + sidx, S - 1 - s);
         __syncthreads();
+        if (pact) {
 #pragma unroll
-        for (int rr = 0; rr < C::RPT; ++rr) {
-            const int prev = __ldcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj);
-            acc[rr] = max(acc[rr], (uint32_t)prev << C::SH);
+            for (int rr = 0; rr < C::RPT; ++rr) {
+                const int prev = __ldcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj);
+                acc[rr] = max(acc[rr], (uint32_t)prev << C::SH);
+            }
         }
     }
+    if (pact) {
 #pragma unroll
-    for (int rr = 0; rr < C::RPT; ++rr)
-        __stcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj, (int16_t)(acc[rr] >> C::SH));
+        for (int rr = 0; rr < C::RPT; ++rr)
+            __stcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj, (int16_t)(acc[rr] >> C::SH));
+    }
     __threadfence();
     __syncthreads();
     if (tid == 0) st_release_gpu(p.accstage + sidx, S - s);
 }
 
 // ------------------------------------------------------------------------------------------------
-// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA): a continuous skewed wavefront
+// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA): one warp per q-tile column
 //
-// Local coordinates: rows a = 0..T-1 (a = T-1 is the bottom row), columns c = 0..T-1.  Lane <-> column:
-// the lane that owns column c walks it bottom-up, one cell per step, one row below its left
-// neighbour: at step k it is on row a = T-1-k+c, so all cells of one anti-diagonal
-// are computed in the same step and the whole tile takes 2T-1 steps, with no barrier between them.
-// CPW = 32/R columns per warp; the R lanes ("roles") of a column hold identical wavefront state and
-// split the table lookups of the step.  Neighbouring warps are coupled by tagged hand-off slots in
-// shared memory (value + row word of the warp's last two columns), polled by the consumer.
+// Local coordinates: rows a = 0..T-1 (a = T-1 is the bottom row), columns c = 0..T-1; the super-tile
+// is 8 x 8 q-tiles (A,B) of Q x Q cells.  Warp B owns q-tile column B and walks it bottom-up,
+// A = 7..0; q-tile (A,B) needs (A+1,B) (the warp's own previous one) and (A,B-1) (warp B-1, awaited
+// through a progress counter in shared memory), so the warps form a skewed pipeline: the q-tiles of
+// one anti-diagonal (7-A)+B run together and the super-tile takes 15 q-tile steps
+// (PAPER.md:223-245 wavefront, PAPER.md:291 tiles of one diagonal are independent).
 //
-// Critical-path split.  Of all candidates of cell (a,c) only two depend on the previous step:
-//   left  = v(a,c-1)  (tail split t = c-1: M(r,c-1) + M(c-1,c), M(c-1,c) = 0)   -- one shuffle
-//   below = v(a+1,c)  (head split t = r+1: M(r,r+1) + M(r+1,c), M(r,r+1) = 0)   -- own register.
-// Everything else of cell (a-1,c) -- the bulk maximum, b + D(i+1,j-1) and every
-// lookup over rows >= a+1 and columns <= c-2 -- is computed during step k ("OLDX") and only enters
-// v(a-1,c) at step k+1.  So the dependent chain of a step is  shuffle -> max.
-//
-// Lookups of one step, target cell (a-1,c).  With the word arrays indexed by z = 0..15 (z < 8: group
-// z of block I, z >= 8: group z-8 of block J) the groups to look up are one contiguous range
-// z = zL..zR,  zL = floor((a+1)/Q),  zR = 8 + floor((c-2)/Q):
-//   z = zL  head special: the running column word Xp (rows >= a+1 of the lane's own column) with the
-//           row word of (I,I)                                 -- the paper's head residual loop
-//   z = zR  tail special: the row word of row a-1 through column c-2 (from lane c-2, by shuffle) with
-//           the column word of (J,J)                          -- the paper's tail residual loop
-//   zL < z < zR  interior: both words complete, read from shared memory (full groups)
-// (PAPER.md:145-155 residual loops as masked lookups: DESIGN.md 4.3).  Words that are not complete yet
-// are zero (the arrays are cleared per tile), and a zero word only yields a valid lower bound, so the
-// walk over the interior may overshoot without harm; its trip count is warp-uniform.
-// DIAG (I == J): row and column words are both the tile's own; only z < 8 is used (zR = floor((c-2)/Q)),
-// plus the merged lookup (row word through c-2, Xp) when zL == zR; cells with c-a <= 1 are 0.
+// Per q-tile, two phases:
+//  (M) mini-products, all 32 lanes: every group that is complete for the whole q-tile -- z in
+//      [A+1, 7] of block I (column words of the q-tiles below, row words of (I,I)) and z in [8, 8+B-1]
+//      of block J (row words of the q-tiles to the left, column words of (J,J)) -- is one lookup per
+//      cell (full groups), merged into val[][].
+//  (C) cell wavefront, lane y <-> column BQ+y, 2Q skewed steps, lane y one row below lane y-1.  Of all
+//      candidates of cell (a,c) only two depend on the previous step:
+//        left  = v(a,c-1)  (tail split t = c-1: M(r,c-1) + M(c-1,c), M(c-1,c) = 0)   -- one shuffle
+//        below = v(a+1,c)  (head split t = r+1: M(r,r+1) + M(r+1,c), M(r,r+1) = 0)   -- own register.
+//      Everything else of the NEXT cell (a-1,c) -- val (bulk + mini-products), b + D(i+1,j-1)
+//      (PAPER.md:135), the head lookup (running column word Xp over rows >= a+1 of the q-tile with the
+//      row word of group A of block I) and the tail lookup (row word of row a-1 through column c-2,
+//      from lane y-2, with the column word of group B of block J) -- is computed during the step
+//      ("oldx") and enters v(a-1,c) one step later: the dependent chain of a step is shuffle -> max.
+//      Head and tail are the paper's residual loops done as masked
+//      lookups: not yet known difference bits are zero (DESIGN.md 4.3 proves this is exact).
+// DIAG (I == J): row and column words are both the tile's own (z < 8 only); warp B starts at A = B;
+// in q-tile (B,B) head and tail are ONE lookup (row word through c-2, Xp); cells with c-a <= 1 are 0.
 // ------------------------------------------------------------------------------------------------
-constexpr uint32_t E_TAG = 0x5a5a0000u;
-
-__device__ __forceinline__ uint2 lds_volatile_u2(const uint2 *p)
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
 {
-    uint2 r;
-    asm volatile("ld.volatile.shared.v2.u32 {%0, %1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(smem_addr(p)) : "memory");
-    return r;
+    asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void sts_volatile_u2(uint2 *p, uint32_t x, uint32_t y)
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
-    asm volatile("st.volatile.shared.v2.u32 [%0], {%1, %2};" ::"r"(smem_addr(p)), "r"(x), "r"(y) : "memory");
+    asm volatile("mbarrier.arrive.release.cta.shared.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.acquire.cta.shared.b64 P1, [%0], %1;\n"
+        "@P1 bra.uni WAIT_DONE;\n"
+        "bra.uni WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
 }
 
 template <int Q>
-__device__ __forceinline__ uint32_t lookup_tagged(const Smem<Q> &sm, uint32_t W, uint32_t X)
+__device__ __forceinline__ uint32_t lookup_tagged(const Smem<Q> &sm, uint32_t S)
 {
-    const uint32_t S = W + X;
     return S + (tbl_gather<Q>(sm, S) << Cfg<Q>::SH);      // (value << SH) | harmless low bits
 }
 
-template <int Q, bool DIAG>
-__device__ __forceinline__ void wave_closure(const Smem<Q> &sm, int cw, int lane)
+// (M) phase of q-tile (A,B): complete groups z in [zlo, zhi], all 32 lanes
+template <int Q>
+__device__ __forceinline__ void qtile_mini(const Smem<Q> &sm, int A, int B, int zlo, int zhi, int lane)
 {
     using C = Cfg<Q>;
-    constexpr int T = C::T, TP = C::TP, VP = C::VP, SH = C::SH, HB = C::HB, R = C::R, CPW = C::CPW, NCW = C::NCW;
-    constexpr uint32_t FULL = 0xffffffffu;
-    constexpr int OFFQ = 64 * Q;                         // keeps the operand of the constant divisions positive
-    const int j = lane % CPW, rho = lane / CPW;
-    const int c = cw * CPW + j;                          // my column (>= T: idle lane, never stores)
-    const bool colok = c < T;
-    const int b = c % Q, B = c / Q;
-    const int zR = (DIAG ? 0 : 8) + (c >= 2 ? (c - 2) / Q : 0);
-    const uint32_t w2keep = (c >= 2) ? FULL : 0u;
-    const int want = 3 - (int)sm.codeC[colok ? c : 0];   // row code that pairs with my column (code 4 -> never)
-    const int B0c = sm.val[T * VP + c + 1];              // bottom edge M((I+1)T, c)
-    const uint32_t XR = DIAG ? 0u : sm.Xst[zR * TP + c]; // static column word of (J,J) for the tail special
-    const int shb = HB + (b > 0 ? b - 1 : 0);            // position of my horizontal difference bit
-    uint2 *E1 = sm.E + (size_t)(2 * cw) * C::ESLOTS, *E2 = E1 + C::ESLOTS;             // slots I produce
-    const uint2 *P1 = sm.E + (size_t)(2 * (cw > 0 ? cw - 1 : 0)) * C::ESLOTS, *P2 = P1 + C::ESLOTS;   // slots I consume
-    const int k0 = cw * CPW - 1;                         // pre-step of my first column
-    const int kstart = DIAG ? max(k0, T) : k0;
-    const int kend = min(T - 1 + (cw + 1) * CPW - 1, 2 * T - 2);
-    const bool r0 = (rho == 0);
-
-    int vout = 0, vprev = 0, oldx = 0;
-    uint32_t wout = 0, Xp = 0;
-#pragma unroll 1
-    for (int k = kstart; k <= kend; ++k) {
-        const int a = T - 1 - k + c;
-        const int d = k - (T - 1);                       // c - a, the same for every lane
-        // ---- receive from the left
-        int Lv = __shfl_up_sync(FULL, vout, 1, CPW);                // v(a, c-1)
-        uint32_t Lw = __shfl_up_sync(FULL, wout, 1, CPW);           // row a   through column c-1
-        uint32_t Lw2 = __shfl_up_sync(FULL, wout, 2, CPW);          // row a-1 through column c-2
-        if (cw == 0) {
-            if (j == 0) Lv = sm.val[a * VP];                        // left edge (a = T: the corner)
-            if (j < 2) Lw2 = 0;
-        } else {
-            const int a0 = T - 1 - k + cw * CPW;                    // row of my first column, warp-uniform
-            uint2 e1 = make_uint2(0u, 0u), e2 = make_uint2(0u, 0u);
-            if (!(DIAG && k == T)) {                                // DIAG: step T-1 is not run, its cells are 0
-                if (a0 >= 0)
-                    for (;;) { e1 = lds_volatile_u2(P1 + a0); if (__all_sync(FULL, (e1.x & 0xffff0000u) == E_TAG)) break; }
-                if (a0 >= 1)
-                    for (;;) { e2 = lds_volatile_u2(P2 + a0 - 1); if (__all_sync(FULL, (e2.x & 0xffff0000u) == E_TAG)) break; }
-            }
-            if (j == 0) { Lv = (int)(e1.x & 0xffffu); Lw = e1.y; Lw2 = e2.y; }
-            if (j == 1) Lw2 = e1.y;
+    constexpr int TP = C::TP, VP = C::VP, SH = C::SH;
+    constexpr int RS = (32 / Q > Q) ? Q : 32 / Q;        // row slots
+    constexpr int NX = (Q + RS - 1) / RS;                // rows per lane
+    const int my = lane % Q, xr = lane / Q;
+    if (zlo > zhi || xr >= RS) return;
+    const int mc = B * Q + my;
+    const int abot = A * Q + Q - 1;
+    uint32_t best[NX];
+#pragma unroll
+    for (int i = 0; i < NX; ++i) best[i] = 0;
+#pragma unroll 2
+    for (int z = zlo; z <= zhi; ++z) {
+        const uint32_t X = sm.Xst[z * TP + mc];
+#pragma unroll
+        for (int i = 0; i < NX; ++i) {
+            const int x = xr + i * RS;
+            const int a = abot - (x < Q ? x : 0);
+            best[i] = max(best[i], lookup_tagged<Q>(sm, sm.Wst[z * TP + a] + X));
         }
+    }
+#pragma unroll
+    for (int i = 0; i < NX; ++i) {
+        const int x = xr + i * RS;
+        if (x < Q) {
+            int16_t *cell = sm.val + (abot - x) * VP + mc + 1;
+            *cell = (int16_t)max((int)*cell, (int)(best[i] >> SH));
+        }
+    }
+}
+
+// (C) phase of q-tile (A,B): 2Q unrolled skewed steps; every address is lane base + immediate.
+// MERGED: q-tile (B,B) of a diagonal super-tile (head and tail are one lookup; c-a = s-Q+1 for every lane).
+template <int Q, bool DIAG, bool MERGED>
+__device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr int TP = C::TP, VP = C::VP, SH = C::SH, HB = C::HB;
+    constexpr uint32_t FULL = 0xffffffffu;
+    constexpr int ZOFF = DIAG ? 0 : 8;
+    const int y = lane % Q;                              // lanes >= Q shadow lane y and store nothing
+    const bool own = lane < Q;
+    const bool firstcol = (y == 0), lastcol = (y == Q - 1);
+    const int src1 = firstcol ? lane : lane - 1, src2 = (y >= 2) ? lane - 2 : lane;
+    const uint32_t w2mask = (y >= 2) ? FULL : 0u;
+    const int c = B * Q + y;
+    const int abot = A * Q + Q - 1;
+    const int shb = HB + (y > 0 ? y - 1 : 0);            // position of my horizontal difference bit
+    const int sh0 = Q - 1 + y;                           // vertical bit of row x = s-y sits at sh0 - s
+    const uint32_t XJ = MERGED ? 0u : sm.Xst[(ZOFF + B) * TP + c];
+    uint32_t pms = 0;                                    // bit (x + y) <-> row x pairs with my column
+    {
+        const int want = 3 - (int)sm.codeC[c];
+#pragma unroll
+        for (int x = 0; x < Q; ++x) pms |= (uint32_t)((int)sm.codeR[abot - x] == want) << x;
+        pms <<= y;
+    }
+    int16_t *vb = sm.val + (abot + y) * VP + c + 1;                 // vb[-s*VP]  = val[a][c],  a = abot + y - s
+    const uint32_t *wb = sm.Wst + A * TP + abot + y - 1;            // wb[-s]     = Wst[A][a-1]
+    uint32_t *wo = sm.Wst + (ZOFF + B) * TP + abot + y;             // wo[-s]     = own row word of row a
+    int vprev = 0, oldx = 0;
+    uint32_t wout = 0, xbits = 0, vsh = 0;
+#pragma unroll
+    for (int s = -1; s <= 2 * Q - 2; ++s) {
+        const int x_lo = s - (Q - 1);                               // rows touched this step: x in [x_lo, s]
+        // ---- receive from the left
+        int Lv = __shfl_sync(FULL, vprev, src1);                    // v(a, c-1)
+        const uint32_t Lw = __shfl_sync(FULL, wout, src1);          // row a   through column c-1
+        const uint32_t Lw2 = __shfl_sync(FULL, wout, src2) & w2mask;   // row a-1 through column c-2
+        if (firstcol) Lv = vb[-s * VP - 1];                         // column c-1 belongs to the q-tile on the left
         // ---- the cell (a3 init + a5 fresh splits)
         int v = max(max(oldx, vprev), Lv);
-        if (a == T) v = B0c;                                        // pre-step: the cell below the tile
-        if (DIAG && d <= 1) v = 0;                                  // D(i,i) = D(i,i-1) = 0
-        const bool live = colok && (unsigned)a < (unsigned)T;
-        if (live && r0) sm.val[a * VP + c + 1] = (int16_t)v;
+        if (s + 1 < Q && y == s + 1) v = vb[-s * VP];               // pre-step (x = -1): the cell below the q-tile
+        if (MERGED && s - (Q - 1) <= 1) v = 0;                      // D(i,i) = D(i,i-1) = 0
+        const bool live = own && (unsigned)(s - y) < (unsigned)Q;
+        if (live) vb[-s * VP] = (int16_t)v;
         // ---- step a6, horizontal: my row word = neighbour's word | my difference bit
-        const uint32_t wme = (b == 0) ? ((uint32_t)v << SH) : (Lw | ((uint32_t)(v - Lv) << shb));
-        if (live && r0 && b == Q - 1) {
-            sm.Wst[(8 + B) * TP + a] = wme;
-            if (DIAG) sm.Wst[B * TP + a] = wme;
+        const uint32_t vnew = (uint32_t)v << SH;
+        const uint32_t wme = firstcol ? vnew : (Lw | ((uint32_t)(v - Lv) << shb));
+        if (live && lastcol) {
+            wo[-s] = wme;
+            if (DIAG) wo[-s + 8 * TP] = wme;
         }
-        if (cw < NCW - 1 && r0 && colok && (unsigned)a <= (unsigned)T) {
-            if (j == CPW - 1) sts_volatile_u2(E1 + a, E_TAG | (uint32_t)(v & 0xffff), wme);
-            if (j == CPW - 2) sts_volatile_u2(E2 + a, E_TAG, wme);
-        }
-        // ---- OLDX of the next cell (a-1, c)
-        int o = sm.val[(a - 1) * VP + c + 1];                       // bulk maximum
-        if ((int)sm.codeR[a - 1] == want) o = max(o, Lv + 1);       // b(S_i,S_j) + D(i+1,j-1)
-        const int zL = min((int)((unsigned)(a + 1 + OFFQ) / Q) - 64, 7);   // floor((a+1)/Q); 7 when no row of the tile is below
-        const int fl = (int)((unsigned)(d - 3 + OFFQ) / Q) - 64;    // floor((d-3)/Q), warp-uniform
-        // warp-uniform upper bound of the interior count zR-zL-1: floor differences give 8+fl; one more because
-        // zR is one too high for columns 0,1 (no tail group) and zL is clamped on the bottom row
-        const int nint = min(DIAG ? fl : 9 + fl, DIAG ? 6 : 14);
-        const int nit = nint > 0 ? (nint + R - 1) / R : 0;
-        const uint32_t Wh = sm.Wst[zL * TP + a - 1];
-        const uint32_t Xt = DIAG ? sm.Xst[zR * TP + c] : XR;
-        const uint32_t Lw2m = Lw2 & w2keep;
+        // ---- oldx of the next cell (a-1, c)
+        int o = vb[-(s + 1) * VP];                                  // bulk + mini-products
+        o = max(o, Lv + (int)((pms >> ((s + 1) & 31)) & 1u));       // b(S_i,S_j) + D(i+1,j-1)
         uint32_t best;
-        if (R == 1) {
-            best = max(lookup_tagged<Q>(sm, Wh, Xp), lookup_tagged<Q>(sm, Lw2m, Xt));
+        uint32_t Xp = xbits + vsh;                                  // running column word: rows >= a+1
+        if (s + 1 < Q && y > s) Xp = 0;                             // not in the q-tile yet: no row of it lies below
+        if (MERGED) {
+            best = lookup_tagged<Q>(sm, Lw2 + Xp);
         } else {
-            const uint32_t W0 = (rho == 0) ? Wh : (rho == 1 ? Lw2m : 0u);
-            const uint32_t X0 = (rho == 0) ? Xp : (rho == 1 ? Xt : 0u);
-            best = lookup_tagged<Q>(sm, W0, X0);
+            best = max(lookup_tagged<Q>(sm, wb[-s] + Xp), lookup_tagged<Q>(sm, Lw2 + XJ));
         }
-        if (DIAG) best = max(best, lookup_tagged<Q>(sm, (zL == zR) ? Lw2m : 0u, Xp));
-        {
-            const uint32_t *pw = sm.Wst + (zL + 1 + rho) * TP + a - 1;
-            const uint32_t *px = sm.Xst + (zL + 1 + rho) * TP + c;
-            constexpr int NITMAX = ((DIAG ? 6 : 14) + R - 1) / R;
-#pragma unroll
-            for (int i = 0; i < NITMAX; ++i) {
-                if (i < nit) best = max(best, lookup_tagged<Q>(sm, pw[i * R * TP], px[i * R * TP]));
-            }
-        }
-        if (R >= 2) best = max(best, __shfl_xor_sync(FULL, best, CPW));
-        if (R >= 4) best = max(best, __shfl_xor_sync(FULL, best, 2 * CPW));
         oldx = max(o, (int)(best >> SH));
-        // ---- step a6, vertical: the column word now starts at row a
-        const int am = (int)((unsigned)(a + OFFQ) % Q);
-        if (a >= T) {
-            Xp = 0;                                                 // nothing of my column is known below the tile
-        } else {
-            Xp = (am == Q - 1) ? ((uint32_t)v << SH)
-                               : ((Xp & C::IDXMASK) | ((uint32_t)(v - vprev) << am) | ((uint32_t)v << SH));
-            if (live && r0 && am == 0) sm.Xst[(a / Q) * TP + c] = Xp;
+        // ---- step a6, vertical: the column word now starts at row a (anchor v, bit of the pair (a, a+1))
+        {
+            const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 0 ? s : 0) & 31);
+            xbits = (y <= s - 1) ? ((xbits | dbit) & C::IDXMASK) : 0u;     // x >= 1
+            vsh = vnew;
         }
-        vprev = v; vout = v; wout = wme;
+        if (x_lo >= 0 && live && y == x_lo) sm.Xst[A * TP + c] = xbits + vsh;    // x = Q-1: the column word is complete
+        vprev = v; wout = wme;
     }
+}
+
+template <int Q, bool DIAG>
+__device__ __forceinline__ void qcol_closure(const Smem<Q> &sm, int B, int lane, uint32_t parity, unsigned long long *prof = nullptr)
+{
+    long long t_poll = 0, t_mini = 0, t_wave = 0, t0 = 0;
+    constexpr int ZOFF = DIAG ? 0 : 8;
+    const int Astart = DIAG ? B : 7;
+    if (DIAG && lane == 0)
+        for (int A = B + 1; A < 8; ++A) mbar_arrive(sm.mbar + B * 8 + A);      // q-tiles below the diagonal: nothing to do
+#pragma unroll 1
+    for (int A = Astart; A >= 0; --A) {
+        if (prof) t0 = clock64();
+        // ---- wait until warp B-1 has finished q-tile (A, B-1)
+        if (B > 0) mbar_wait(sm.mbar + (B - 1) * 8 + A, parity);
+        __syncwarp();
+        if (prof) { const long long t1 = clock64(); t_poll += t1 - t0; t0 = t1; }
+        qtile_mini<Q>(sm, A, B, A + 1, ZOFF + B - 1, lane);
+        __syncwarp();
+        if (prof) { const long long t1 = clock64(); t_mini += t1 - t0; t0 = t1; }
+        if (DIAG && A == B) qtile_wave<Q, true, true>(sm, A, B, lane);
+        else qtile_wave<Q, DIAG, false>(sm, A, B, lane);
+        // ---- publish the q-tile to warp B+1
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.mbar + B * 8 + A);
+        if (prof) { const long long t1 = clock64(); t_wave += t1 - t0; t0 = t1; }
+    }
+    if (prof && lane == 0)
+        prof[0] = ((unsigned long long)(t_poll & 0x1fffff)) | ((unsigned long long)(t_mini & 0x1fffff) << 21) | ((unsigned long long)(t_wave & 0x1fffff) << 42);
 }
 
 // ---- CLOSE task ----
@@ -603,14 +637,13 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
     }
 
     const int warp = tid >> 5, lane = tid & 31;
-    // hand-off slots of the wavefront warps: empty
-    for (int e = tid; e < C::E_BYTES / 8; e += C::NTHR) sm.E[e] = make_uint2(0u, 0u);
+    const uint32_t parity = (uint32_t)sm.misc[1] & 1u;    // closures this CTA has run so far: phase of the q-tile mbarriers
     if (dp == 0) {
         // diagonal super-tile: everything starts from zero
-        for (int e = tid; e < C::VAL_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.val)[e] = 0;
+        for (int e = tid; e < C::VAL_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.valraw)[e] = 0;
         for (int e = tid; e < C::WROWS * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
         __syncthreads();
-        if (warp < C::NCW) wave_closure<Q, true>(sm, warp, lane);
+        if (warp < 8) qcol_closure<Q, true>(sm, warp, lane, parity, (tr && warp == 7) ? tr + 7 : nullptr);
         __syncthreads();
     } else {
         const int s_left = si.sbase + tri_index(nt, I, J - 1);
@@ -636,10 +669,8 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
                 sm.Wst[g * C::TP + k] = __ldcg(ph + e);
                 sm.Xst[(8 + g) * C::TP + k] = __ldcg(pv + e);
             }
-            // the tile's own words are not known yet: zero (= a valid lower bound); zero guard rows
-            for (int e = tid; e < (C::WROWS - 8) * C::TP; e += C::NTHR) sm.Wst[8 * C::TP + e] = 0;
-            for (int e = tid; e < 8 * C::TP; e += C::NTHR) sm.Xst[e] = 0;
-            for (int e = tid; e < (C::WROWS - 16) * C::TP; e += C::NTHR) sm.Xst[16 * C::TP + e] = 0;
+            // the tile's own words are not known yet: zero (= a valid lower bound)
+            for (int e = tid; e < 8 * C::TP; e += C::NTHR) { sm.Wst[8 * C::TP + e] = 0; sm.Xst[e] = 0; }
         }
         // bulk maxima gathered by the PROD stages (or zero)
         if (S > 0) {
@@ -671,7 +702,8 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         if (tr && tid == 0) tr[2] = global_timer_ns();
         // late products: the middle blocks whose panels were only finished on the previous step
         if (dp >= 2) {
-            const int jj = tid % T, rb = tid / T;
+            const bool pact = tid < C::PTHR;
+            const int jj = tid % T, rb = pact ? tid / T : 0;
             uint32_t acc[C::RPT];
 #pragma unroll
             for (int rr = 0; rr < C::RPT; ++rr) acc[rr] = 0;
@@ -684,21 +716,23 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
                 cp_async_wait<0>();
             }
             __syncthreads();
-            product_accumulate<Q>(sm, 0, acc, jj, rb);
+            if (pact) product_accumulate<Q>(sm, 0, acc, jj, rb);
             if (K1 != K0) {
                 cp_async_wait<0>();
                 __syncthreads();
-                product_accumulate<Q>(sm, 1, acc, jj, rb);
+                if (pact) product_accumulate<Q>(sm, 1, acc, jj, rb);
             }
+            if (pact) {
 #pragma unroll
-            for (int rr = 0; rr < C::RPT; ++rr) {
-                int16_t *cell = sm.val + (rb * C::RPT + rr) * C::VP + jj + 1;
-                *cell = (int16_t)max((int)*cell, (int)(acc[rr] >> C::SH));
+                for (int rr = 0; rr < C::RPT; ++rr) {
+                    int16_t *cell = sm.val + (rb * C::RPT + rr) * C::VP + jj + 1;
+                    *cell = (int16_t)max((int)*cell, (int)(acc[rr] >> C::SH));
+                }
             }
             __syncthreads();
         }
         if (tr && tid == 0) tr[3] = global_timer_ns();
-        if (warp < C::NCW) wave_closure<Q, false>(sm, warp, lane);
+        if (warp < 8) qcol_closure<Q, false>(sm, warp, lane, parity, (tr && warp == 7) ? tr + 7 : nullptr);
         __syncthreads();
     }
     if (tr && tid == 0) tr[4] = global_timer_ns();
@@ -735,7 +769,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
         __threadfence();
         __syncthreads();
-        if (tid == 0) { st_release_gpu(p.done + sidx, 1); if (tr) tr[5] = global_timer_ns(); }
+        if (tid == 0) { st_release_gpu(p.done + sidx, 1); sm.misc[1] += 1; if (tr) tr[5] = global_timer_ns(); }
     }
 }
 
@@ -754,6 +788,8 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR) fill_kernel(Params p)
         for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
         if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
     }
+    if (tid < 64) mbar_init(sm.mbar + tid, 1);
+    if (tid == 0) sm.misc[1] = 0;
     __syncthreads();
     const int total = p.hdr->total;
     for (;;) {
