@@ -143,7 +143,7 @@ class Rna4r:
         _check(self.lib.rna4r_set_trace(self.h, int(max_tiles)), "rna4r_set_trace")
 
     def trace(self, tiles: int) -> np.ndarray:
-        out = np.zeros((tiles, 8), dtype=np.uint64)
+        out = np.zeros((tiles, int(os.environ.get("RNA4R_TRACE_WORDS", "8"))), dtype=np.uint64)
         _check(self.lib.rna4r_trace_to_host(self.h, out.ctypes.data, tiles), "rna4r_trace_to_host")
         return out
 

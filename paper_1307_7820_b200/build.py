@@ -30,7 +30,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB, os.path.join(HERE, "csrc", "api.cu")]
+    extra = os.environ.get("RNA4R_NVCC_FLAGS", "").split()          # tuning builds only (e.g. -DRNA4R_TRACE_WORDS=256)
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB, os.path.join(HERE, "csrc", "api.cu")]
     subprocess.check_call(cmd)
     return LIB
 

@@ -167,8 +167,8 @@ int rna4r_set_trace(rna4r_ctx *ctx, int max_tiles)
     cudaFree(ctx->trace);
     ctx->trace = nullptr; ctx->trace_tiles = 0;
     if (max_tiles > 0) {
-        RNA4R_CUDA(ctx, cudaMalloc(&ctx->trace, (size_t)max_tiles * 64));
-        RNA4R_CUDA(ctx, cudaMemset(ctx->trace, 0, (size_t)max_tiles * 64));
+        RNA4R_CUDA(ctx, cudaMalloc(&ctx->trace, (size_t)max_tiles * 8 * RNA4R_TRACE_WORDS));
+        RNA4R_CUDA(ctx, cudaMemset(ctx->trace, 0, (size_t)max_tiles * 8 * RNA4R_TRACE_WORDS));
         ctx->trace_tiles = max_tiles;
     }
     return RNA4R_OK;
@@ -181,7 +181,7 @@ int rna4r_trace_to_host(rna4r_ctx *ctx, uint64_t *dst_host, int tiles)
     if (!ctx->trace || tiles < 0 || tiles > ctx->trace_tiles) return RNA4R_ERR_BAD_N;
     RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
     RNA4R_CUDA(ctx, cudaDeviceSynchronize());
-    RNA4R_CUDA(ctx, cudaMemcpy(dst_host, ctx->trace, (size_t)tiles * 64, cudaMemcpyDeviceToHost));
+    RNA4R_CUDA(ctx, cudaMemcpy(dst_host, ctx->trace, (size_t)tiles * 8 * RNA4R_TRACE_WORDS, cudaMemcpyDeviceToHost));
     return RNA4R_OK;
 }
 

@@ -23,6 +23,11 @@ struct rna4r_ctx {
     unsigned long long *trace;   // optional per-super-tile phase stamps (rna4r_set_trace)
     int trace_tiles;
 };
+// u64 words per super-tile in the optional trace buffer (rna4r_set_trace); a build with
+// -DRNA4R_TRACE_WORDS=256 adds per-q-tile event stamps for tuning
+#ifndef RNA4R_TRACE_WORDS
+#define RNA4R_TRACE_WORDS 8
+#endif
 static const uint32_t RNA4R_MAGIC = 0x52344e41u;
 
 #define RNA4R_CUDA(ctx, call)                                             \

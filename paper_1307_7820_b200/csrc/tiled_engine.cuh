@@ -46,7 +46,9 @@ struct Cfg {
     static constexpr bool TBL_ALIGNED = (Q <= 8);
     static constexpr int TBL_ALIGN = TBL_ALIGNED ? (TBL_BYTES < 16 ? 16 : TBL_BYTES) : 16;
     static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
-    static constexpr int NTHR = PTHR > 256 ? PTHR : 256;   // threads per CTA: at least the 8 closure warps
+    static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
+    static constexpr int NTHR = WTHR + 128;    // + 4 helper warps of the closure: loader, publisher, 2 x late products
+    static constexpr int HW0 = WTHR / 32;      // first helper warp
     static constexpr int RPT = 2 * Q;          // rows per thread in the product phase
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
     static constexpr int VP = T + 1;           // pitch of the value array (int16): a wavefront step is conflict-free
@@ -62,8 +64,14 @@ struct Cfg {
     static constexpr int VAL_ROWS = T + 1 + 2 * Q;   // Q guard rows, rows 0..T, Q guard rows
     static constexpr int VAL_BYTES = ((VAL_ROWS * VP + 2) * 2 + 15) / 16 * 16;
     static constexpr int STG_BYTES = 2 * 2 * PANEL_WORDS * 4;
-    static constexpr int MBAR_BYTES = 64 * 8;  // one mbarrier per q-tile: warp B -> warp B+1 hand-off
-    static constexpr int POST_BYTES = VAL_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
+    static constexpr int VP2 = T + 2;          // pitch of val2 (int16): odd word stride, a column of it is conflict-free
+    static constexpr int VAL2_BYTES = (T * VP2 * 2 + 15) / 16 * 16;   // late products of block I+1 (kept apart: two warps merge concurrently)
+    // mbarriers (each completes once per closure): [0,64) q-tile (A,B) done, at B*8+A; [64,72) rows of q-row A
+    // of the left tile loaded; [72,80) columns of q-column B of the tile below loaded; [80,88) late products of
+    // q-row A merged; [88,96) late products of q-column B merged
+    static constexpr int MB_ROW = 64, MB_COL = 72, MB_RLATE = 80, MB_CLATE = 88, MB_COUNT = 96;
+    static constexpr int MBAR_BYTES = MB_COUNT * 8;
+    static constexpr int POST_BYTES = VAL_BYTES + VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
     // dynamic shared memory needed when the dynamic window starts at shared address `base`
     static constexpr size_t smem_bytes_for(size_t base)
     {
@@ -109,6 +117,8 @@ struct Params {
     SeqInfo *seqinfo; // [count]
     int *done;        // [tiles] 1 when the super-tile's panels are published
     int *accstage;    // [tiles] product stages merged into acc so far
+    int *rowprog;     // [tiles] q-rows (from the bottom) whose row words and right-column values are published
+    int *colprog;     // [tiles] q-columns (from the left) whose column words and top-row values are published
     int4 *tasks;      // {seq, I | J << 16, kind, stage}
     int8_t *codes;    // per sequence nt*T codes (4 = padding)
     uint8_t *recs;    // super-tile records
@@ -228,6 +238,7 @@ struct Smem {
     uint32_t tbl_sa;     // its shared-space address (aligned to TBL_ALIGN)
     int16_t *valraw;     // start of the value array including its guard rows
     int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
+    int16_t *val2;       // [T][VP2] late products of block K = I+1 (written by the column-late helper, merged by the closure warps)
     uint32_t *stg;       // [2][2][PANEL_WORDS] product operands, double buffered: [buf][0]=PH, [buf][1]=PV
     int8_t *codeR;       // [T] codes of the rows
     int8_t *codeC;       // [T] codes of the columns
@@ -245,6 +256,7 @@ struct Smem {
         p = base + (tsa - sa0);
         tbl = p; tbl_sa = tsa; p += (C::TBL_BYTES + 15) / 16 * 16;
         valraw = (int16_t *)p; val = valraw + Q * C::VP; p += C::VAL_BYTES;     // val[0] = row 0; Q guard rows on either side
+        val2 = (int16_t *)p; p += C::VAL2_BYTES;
         stg = (uint32_t *)p; p += C::STG_BYTES;
         codeR = (int8_t *)p; p += C::T;
         codeC = (int8_t *)p; p += C::T;
@@ -477,16 +489,19 @@ __device__ __forceinline__ uint32_t lookup_tagged(const Smem<Q> &sm, uint32_t S)
     return S + (tbl_gather<Q>(sm, S) << Cfg<Q>::SH);      // (value << SH) | harmless low bits
 }
 
-// (M) phase of q-tile (A,B): complete groups z in [zlo, zhi], all 32 lanes
+// Complete-group lookups for the Q x Q cells of q-tile (A,B), all 32 lanes: for z in [zlo, zhi],
+// val[a][c] = max(val[a][c], lookup(W[z*wp + a] + X[z*xp + c])).  Used for the mini-products of the
+// closure (W = Wst, X = Xst) and for the late products (operand panels of the neighbouring blocks).
 template <int Q>
-__device__ __forceinline__ void qtile_mini(const Smem<Q> &sm, int A, int B, int zlo, int zhi, int lane)
+__device__ __forceinline__ void qtile_groups(const Smem<Q> &sm, int A, int B, const uint32_t *W, int wp, const uint32_t *X, int xp,
+                                             int zlo, int zhi, int lane, bool merge2 = false)
 {
     using C = Cfg<Q>;
-    constexpr int TP = C::TP, VP = C::VP, SH = C::SH;
+    constexpr int VP = C::VP, SH = C::SH;
     constexpr int RS = (32 / Q > Q) ? Q : 32 / Q;        // row slots
     constexpr int NX = (Q + RS - 1) / RS;                // rows per lane
     const int my = lane % Q, xr = lane / Q;
-    if (zlo > zhi || xr >= RS) return;
+    if ((zlo > zhi && !merge2) || xr >= RS) return;
     const int mc = B * Q + my;
     const int abot = A * Q + Q - 1;
     uint32_t best[NX];
@@ -494,12 +509,12 @@ __device__ __forceinline__ void qtile_mini(const Smem<Q> &sm, int A, int B, int 
     for (int i = 0; i < NX; ++i) best[i] = 0;
 #pragma unroll 2
     for (int z = zlo; z <= zhi; ++z) {
-        const uint32_t X = sm.Xst[z * TP + mc];
+        const uint32_t Xw = X[z * xp + mc];
 #pragma unroll
         for (int i = 0; i < NX; ++i) {
             const int x = xr + i * RS;
             const int a = abot - (x < Q ? x : 0);
-            best[i] = max(best[i], lookup_tagged<Q>(sm, sm.Wst[z * TP + a] + X));
+            best[i] = max(best[i], lookup_tagged<Q>(sm, W[z * wp + a] + Xw));
         }
     }
 #pragma unroll
@@ -507,7 +522,9 @@ __device__ __forceinline__ void qtile_mini(const Smem<Q> &sm, int A, int B, int 
         const int x = xr + i * RS;
         if (x < Q) {
             int16_t *cell = sm.val + (abot - x) * VP + mc + 1;
-            *cell = (int16_t)max((int)*cell, (int)(best[i] >> SH));
+            int v = max((int)*cell, (int)(best[i] >> SH));
+            if (merge2) v = max(v, (int)sm.val2[(abot - x) * C::VP2 + mc]);      // late products of block I+1
+            *cell = (int16_t)v;
         }
     }
 }
@@ -587,33 +604,218 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
     }
 }
 
-template <int Q, bool DIAG>
-__device__ __forceinline__ void qcol_closure(const Smem<Q> &sm, int B, int lane, uint32_t parity, unsigned long long *prof = nullptr)
+// Operand panels of the late products, in the staging area (pitch T): rows of the left tile (I,J-1),
+// column panel of (J-1,J), row panel of (I,I+1), columns of the tile below (I+1,J).
+template <int Q> __device__ __forceinline__ uint32_t *panel_ZW(const Smem<Q> &sm) { return sm.stg; }
+template <int Q> __device__ __forceinline__ uint32_t *panel_XJ1(const Smem<Q> &sm) { return sm.stg + Cfg<Q>::PANEL_WORDS; }
+template <int Q> __device__ __forceinline__ uint32_t *panel_WI1(const Smem<Q> &sm) { return sm.stg + 2 * Cfg<Q>::PANEL_WORDS; }
+template <int Q> __device__ __forceinline__ uint32_t *panel_YX(const Smem<Q> &sm) { return sm.stg + 3 * Cfg<Q>::PANEL_WORDS; }
+
+struct CloseCtx {
+    int dp;              // J - I
+    uint32_t parity;     // phase of this closure's mbarriers
+    const uint8_t *recZ; // record of the left tile (I,J-1)
+    const uint8_t *recY; // record of the tile below (I+1,J)
+    const uint8_t *recC; // record of the corner tile (I+1,J-1), or NULL (dp < 2: below the diagonal, value 0)
+    uint8_t *recX;       // record of this tile
+    const int *rowprogZ, *colprogY, *doneC;
+    int *rowprogX, *colprogX;
+    unsigned long long *ev;   // fine trace of this closure (RNA4R_TRACE_WORDS > 8), else NULL
+};
+#define RNA4R_EV(cc, idx) do { if (RNA4R_TRACE_WORDS > 8 && (cc).ev && lane == 0) (cc).ev[idx] = global_timer_ns(); } while (0)
+
+__device__ __forceinline__ void warp_wait_flag_ge(const int *flag, int v, int lane)
 {
+    if (lane == 0) { unsigned ns = 20; while (ld_acquire_gpu(flag) < v) { __nanosleep(ns); if (ns < 160) ns *= 2; } }
+    __syncwarp();
+}
+
+// closure warp B (q-tile column B), off-diagonal super-tile and diagonal super-tile
+template <int Q, bool DIAG>
+__device__ __forceinline__ void qcol_closure(const Smem<Q> &sm, const CloseCtx &cc, int B, int lane, unsigned long long *prof = nullptr)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T, TP = C::TP, VP = C::VP;
     long long t_poll = 0, t_mini = 0, t_wave = 0, t0 = 0;
     constexpr int ZOFF = DIAG ? 0 : 8;
     const int Astart = DIAG ? B : 7;
-    if (DIAG && lane == 0)
-        for (int A = B + 1; A < 8; ++A) mbar_arrive(sm.mbar + B * 8 + A);      // q-tiles below the diagonal: nothing to do
+    if (DIAG) {
+        if (lane == 0) for (int A = B + 1; A < 8; ++A) mbar_arrive(sm.mbar + B * 8 + A);      // q-tiles below the diagonal: nothing to do
+    } else {
+        // ---- my columns of the tile below: column words (late products) and its top row (my bottom edge)
+        warp_wait_flag_ge(cc.colprogY, B + 1, lane);
+        const uint32_t *pv = reinterpret_cast<const uint32_t *>(cc.recY) + C::PANEL_WORDS;
+        const uint16_t *etop = reinterpret_cast<const uint16_t *>(cc.recY + 2 * C::PANEL_WORDS * 4);
+        uint32_t *YX = panel_YX<Q>(sm);
+        for (int e = lane; e < 8 * Q; e += 32) {
+            const int g = e / Q, k = B * Q + e % Q;
+            YX[g * T + k] = __ldcg(pv + g * T + k);
+        }
+        if (lane < Q) sm.val[T * VP + B * Q + lane + 1] = (int16_t)__ldcg(etop + B * Q + lane);
+        if (B == 0 && lane == 0) {
+            // corner M((I+1)T, JT-1) = top row of (I+1,J-1) at its last column
+            int corner = 0;
+            if (cc.recC) {
+                while (ld_acquire_gpu(cc.doneC) < 1) __nanosleep(40);
+                corner = __ldcg(reinterpret_cast<const uint16_t *>(cc.recC + 2 * C::PANEL_WORDS * 4) + T - 1);
+            }
+            sm.val[T * VP] = (int16_t)corner;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_COL + B);
+        RNA4R_EV(cc, 144 + B);
+        mbar_wait(sm.mbar + C::MB_CLATE + B, cc.parity);        // late products of my columns
+    }
 #pragma unroll 1
     for (int A = Astart; A >= 0; --A) {
         if (prof) t0 = clock64();
-        // ---- wait until warp B-1 has finished q-tile (A, B-1)
-        if (B > 0) mbar_wait(sm.mbar + (B - 1) * 8 + A, parity);
+        // ---- wait for q-tile (A, B-1) and for the late products (and edges) of (A, B)
+        if (B > 0) mbar_wait(sm.mbar + (B - 1) * 8 + A, cc.parity);
+        if (!DIAG) mbar_wait(sm.mbar + C::MB_RLATE + A, cc.parity);   // left edge and late products of q-row A
         __syncwarp();
+        RNA4R_EV(cc, 72 + B * 8 + A);
         if (prof) { const long long t1 = clock64(); t_poll += t1 - t0; t0 = t1; }
-        qtile_mini<Q>(sm, A, B, A + 1, ZOFF + B - 1, lane);
+        qtile_groups<Q>(sm, A, B, sm.Wst, TP, sm.Xst, TP, A + 1, ZOFF + B - 1, lane, !DIAG && cc.dp >= 3);
         __syncwarp();
         if (prof) { const long long t1 = clock64(); t_mini += t1 - t0; t0 = t1; }
         if (DIAG && A == B) qtile_wave<Q, true, true>(sm, A, B, lane);
         else qtile_wave<Q, DIAG, false>(sm, A, B, lane);
-        // ---- publish the q-tile to warp B+1
+        // ---- hand the q-tile to warp B+1 (and to the publisher)
         __syncwarp();
         if (lane == 0) mbar_arrive(sm.mbar + B * 8 + A);
+        RNA4R_EV(cc, 8 + B * 8 + A);
         if (prof) { const long long t1 = clock64(); t_wave += t1 - t0; t0 = t1; }
     }
     if (prof && lane == 0)
         prof[0] = ((unsigned long long)(t_poll & 0x1fffff)) | ((unsigned long long)(t_mini & 0x1fffff) << 21) | ((unsigned long long)(t_wave & 0x1fffff) << 42);
+}
+
+// helper warp: rows of the left tile, q-row by q-row as it publishes them (row words for the late
+// products, right-column values = my left edge)
+template <int Q>
+__device__ __forceinline__ void close_row_loader(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T, VP = C::VP;
+    const uint32_t *ph = reinterpret_cast<const uint32_t *>(cc.recZ);
+    const uint16_t *eright = reinterpret_cast<const uint16_t *>(cc.recZ + 2 * C::PANEL_WORDS * 4) + T;
+    uint32_t *ZW = panel_ZW<Q>(sm);
+    for (int A = 7; A >= 0; --A) {
+        warp_wait_flag_ge(cc.rowprogZ, 8 - A, lane);
+        for (int e = lane; e < 8 * Q; e += 32) {
+            const int g = e / Q, k = A * Q + e % Q;
+            ZW[g * T + k] = __ldcg(ph + g * T + k);
+        }
+        if (lane < Q) sm.val[(A * Q + lane) * VP] = (int16_t)__ldcg(eright + A * Q + lane);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_ROW + A);
+        RNA4R_EV(cc, 136 + A);
+    }
+}
+
+// helper warp: publishes the tile q-row by q-row and q-column by q-column (step a6 output): row words and
+// right-column values of q-row A once q-tile (A,7) is done, column words and top-row values of q-column B
+// once q-tile (0,B) is done.
+template <int Q>
+__device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T, TP = C::TP, VP = C::VP;
+    uint32_t *ph = reinterpret_cast<uint32_t *>(cc.recX);
+    uint32_t *pv = ph + C::PANEL_WORDS;
+    uint16_t *edge = reinterpret_cast<uint16_t *>(cc.recX + 2 * C::PANEL_WORDS * 4);
+    for (int i = 0; i < 8; ++i) {
+        {
+            const int B = i;
+            mbar_wait(sm.mbar + B * 8 + 0, cc.parity);
+            for (int e = lane; e < 8 * Q; e += 32) {
+                const int g = e / Q, k = B * Q + e % Q;
+                __stcg(pv + g * T + k, sm.Xst[g * TP + k]);
+            }
+            if (lane < Q) __stcg(edge + B * Q + lane, (uint16_t)sm.val[B * Q + lane + 1]);           // top row  M(I*T, c)
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release_gpu(cc.colprogX, B + 1);
+            RNA4R_EV(cc, 224 + B);
+        }
+        {
+            const int A = 7 - i;
+            mbar_wait(sm.mbar + 7 * 8 + A, cc.parity);
+            for (int e = lane; e < 8 * Q; e += 32) {
+                const int g = e / Q, k = A * Q + e % Q;
+                __stcg(ph + g * T + k, sm.Wst[(8 + g) * TP + k]);
+            }
+            if (lane < Q) __stcg(edge + T + A * Q + lane, (uint16_t)sm.val[(A * Q + lane) * VP + T]);   // right column M(r, J*T+T-1)
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release_gpu(cc.rowprogX, 8 - A);
+            RNA4R_EV(cc, 216 + A);
+        }
+    }
+}
+
+// Late products: the two middle blocks K = J-1 and K = I+1 whose panels are only being finished now.
+// One max-plus product of Q rows x T columns (row_late: rows of q-row A of the left tile x column panel of
+// (J-1,J)) or T rows x Q columns (col_late: row panel of (I,I+1) x columns of q-column B of the tile below)
+// over the 8 groups of the block; a lane owns one column (row) and NR rows (columns), so the words of the
+// short side are warp-uniform broadcast loads, as in the bulk product.
+template <int Q>
+__device__ __forceinline__ void late_strip(const Smem<Q> &sm, const uint32_t *U, int u0, const uint32_t *L, int16_t *out, int out_us, int out_ls,
+                                           bool domax, int lane)
+{
+    // U[g*T + u0 + i], i < Q: the uniform side; L[g*T + l], l < T: the lane side; out[(u0+i)*out_us + l*out_ls]
+    using C = Cfg<Q>;
+    constexpr int T = C::T, SH = C::SH;
+    for (int l = lane; l < T; l += 32) {
+        uint32_t acc[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) acc[i] = 0;
+#pragma unroll 2
+        for (int g = 0; g < 8; ++g) {
+            const uint32_t Lw = L[g * T + l];
+            const uint32_t *u = U + g * T + u0;
+#pragma unroll
+            for (int i = 0; i < Q; ++i) acc[i] = max(acc[i], lookup_tagged<Q>(sm, u[i] + Lw));
+        }
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            int16_t *cell = out + (u0 + i) * out_us + l * out_ls;
+            const int v = (int)(acc[i] >> SH);
+            *cell = (int16_t)(domax ? max((int)*cell, v) : v);
+        }
+    }
+}
+
+// helper warp 2: q-row A as soon as the loader has it (rows of the left tile): block K = J-1, into val
+template <int Q>
+__device__ __forceinline__ void close_row_late(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+{
+    using C = Cfg<Q>;
+    if (cc.dp == 2)       // K = J-1 = I+1: both operands arrive now; wait for every column of the tile below
+        for (int B = 0; B < 8; ++B) mbar_wait(sm.mbar + C::MB_COL + B, cc.parity);
+    for (int A = 7; A >= 0; --A) {
+        mbar_wait(sm.mbar + C::MB_ROW + A, cc.parity);
+        if (cc.dp >= 2)
+            late_strip<Q>(sm, panel_ZW<Q>(sm), A * Q, cc.dp == 2 ? panel_YX<Q>(sm) : panel_XJ1<Q>(sm), sm.val + 1, C::VP, 1, true, lane);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_RLATE + A);
+        RNA4R_EV(cc, 152 + A);
+    }
+}
+
+// helper warp 3: q-column B as soon as its closure warp has loaded it (columns of the tile below): block K = I+1, into val2
+template <int Q>
+__device__ __forceinline__ void close_col_late(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+{
+    using C = Cfg<Q>;
+    for (int B = 0; B < 8; ++B) {
+        mbar_wait(sm.mbar + C::MB_COL + B, cc.parity);
+        if (cc.dp >= 3)
+            late_strip<Q>(sm, panel_YX<Q>(sm), B * Q, panel_WI1<Q>(sm), sm.val2, 1, C::VP2, false, lane);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_CLATE + B);
+        RNA4R_EV(cc, 160 + B);
+    }
 }
 
 // ---- CLOSE task ----
@@ -626,7 +828,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
     const int nt = si.nt;
     const int dp = J - I;
     const int sidx = si.sbase + tri_index(nt, I, J);
-    unsigned long long *tr = (p.trace && sidx < p.trace_tiles) ? p.trace + (size_t)sidx * 8 : nullptr;
+    unsigned long long *tr = (p.trace && sidx < p.trace_tiles) ? p.trace + (size_t)sidx * RNA4R_TRACE_WORDS : nullptr;
     if (tr && tid == 0) { tr[0] = global_timer_ns(); tr[6] = ((unsigned long long)I << 32) | (unsigned)J; }
 
     // codes of the rows r = I*T + a (base S[r]) and of the columns c = J*T + jj (base S[c-1])
@@ -635,114 +837,31 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         const int c = J * T + tid;
         sm.codeC[tid] = (c >= 1) ? p.codes[si.cbase + c - 1] : (int8_t)4;
     }
+    // roles by warp, counted from the top: the SM's issue arbiter favours high warp ids, and the closure
+    // warps carry the critical path
+    const int warp = (C::NTHR / 32 - 1) - (tid >> 5), lane = tid & 31;
+    CloseCtx cc;
+    cc.dp = dp;
+    cc.parity = (uint32_t)sm.misc[1] & 1u;    // closures this CTA has run so far: phase of its mbarriers
+    cc.recX = const_cast<uint8_t *>(rec_ptr<Q>(p, sidx));
+    cc.rowprogX = p.rowprog + sidx; cc.colprogX = p.colprog + sidx;
+    cc.ev = (RNA4R_TRACE_WORDS > 8) ? tr : nullptr;
+    cc.recZ = cc.recY = cc.recC = nullptr; cc.rowprogZ = cc.colprogY = cc.doneC = nullptr;
 
-    const int warp = tid >> 5, lane = tid & 31;
-    const uint32_t parity = (uint32_t)sm.misc[1] & 1u;    // closures this CTA has run so far: phase of the q-tile mbarriers
     if (dp == 0) {
-        // diagonal super-tile: everything starts from zero
+        // diagonal super-tile: everything starts from zero; no neighbour, no late product
         for (int e = tid; e < C::VAL_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.valraw)[e] = 0;
         for (int e = tid; e < C::WROWS * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
         __syncthreads();
-        if (warp < 8) qcol_closure<Q, true>(sm, warp, lane, parity, (tr && warp == 7) ? tr + 7 : nullptr);
+        if (warp < 8) qcol_closure<Q, true>(sm, cc, warp, lane, (tr && warp == 7) ? tr + 7 : nullptr);
+        else if (warp == 8)
+            for (int e = lane; e < C::MB_COUNT - C::MB_ROW; e += 32) mbar_arrive(sm.mbar + C::MB_ROW + e);   // keep the phases in step
         __syncthreads();
-    } else {
-        const int s_left = si.sbase + tri_index(nt, I, J - 1);
-        const int s_below = si.sbase + tri_index(nt, I + 1, J);
-        const int s_ii = si.sbase + tri_index(nt, I, I);
-        const int s_jj = si.sbase + tri_index(nt, J, J);
-        const int S = nstages(dp, p.delta);
-        if (tid == 0) {
-            wait_flag_ge(p.done + s_left, 1);
-            wait_flag_ge(p.done + s_below, 1);
-            wait_flag_ge(p.done + s_ii, 1);
-            wait_flag_ge(p.done + s_jj, 1);
-            if (S > 0) wait_flag_ge(p.accstage + sidx, S);
-            if (tr) tr[1] = global_timer_ns();
-        }
-        __syncthreads();
-        // static words: row words of (I,I) -> Wst[0..7], column words of (J,J) -> Xst[8..15]
-        {
-            const uint32_t *ph = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_ii));
-            const uint32_t *pv = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_jj)) + C::PANEL_WORDS;
-            for (int e = tid; e < C::PANEL_WORDS; e += C::NTHR) {
-                const int g = e / T, k = e % T;
-                sm.Wst[g * C::TP + k] = __ldcg(ph + e);
-                sm.Xst[(8 + g) * C::TP + k] = __ldcg(pv + e);
-            }
-            // the tile's own words are not known yet: zero (= a valid lower bound)
-            for (int e = tid; e < 8 * C::TP; e += C::NTHR) { sm.Wst[8 * C::TP + e] = 0; sm.Xst[e] = 0; }
-        }
-        // bulk maxima gathered by the PROD stages (or zero)
-        if (S > 0) {
-            const int16_t *accg = p.acc + (size_t)sidx * T * T;
-            for (int e = tid; e < T * T; e += C::NTHR) sm.val[(e / T) * C::VP + (e % T) + 1] = __ldcg(accg + e);
-        } else {
-            for (int e = tid; e < T * T; e += C::NTHR) sm.val[(e / T) * C::VP + (e % T) + 1] = 0;
-        }
-        // neighbours' edges: right column of (I,J-1) -> val[a][0]; top row of (I+1,J) -> val[T][jj+1];
-        // corner M((I+1)T, JT-1) = top row of (I+1,J-1) at its last column (0 if that tile is below the diagonal)
-        {
-            const uint16_t *eleft = reinterpret_cast<const uint16_t *>(rec_ptr<Q>(p, s_left) + 2 * C::PANEL_WORDS * 4);
-            const uint16_t *ebelow = reinterpret_cast<const uint16_t *>(rec_ptr<Q>(p, s_below) + 2 * C::PANEL_WORDS * 4);
-            if (tid < T) {
-                sm.val[tid * C::VP] = (int16_t)__ldcg(eleft + T + tid);          // right column
-                sm.val[T * C::VP + tid + 1] = (int16_t)__ldcg(ebelow + tid);     // top row
-            }
-            if (tid == T) {
-                int corner = 0;
-                if (dp >= 2) {
-                    const uint16_t *ec = reinterpret_cast<const uint16_t *>(
-                        rec_ptr<Q>(p, si.sbase + tri_index(nt, I + 1, J - 1)) + 2 * C::PANEL_WORDS * 4);
-                    corner = __ldcg(ec + T - 1);
-                }
-                sm.val[T * C::VP] = (int16_t)corner;
-            }
-        }
-        __syncthreads();
-        if (tr && tid == 0) tr[2] = global_timer_ns();
-        // late products: the middle blocks whose panels were only finished on the previous step
-        if (dp >= 2) {
-            const bool pact = tid < C::PTHR;
-            const int jj = tid % T, rb = pact ? tid / T : 0;
-            uint32_t acc[C::RPT];
-#pragma unroll
-            for (int rr = 0; rr < C::RPT; ++rr) acc[rr] = 0;
-            const int K0 = I + 1, K1 = J - 1;
-            load_operands_async<Q>(p, sm, 0, si.sbase + tri_index(nt, I, K0), si.sbase + tri_index(nt, K0, J));
-            if (K1 != K0) {
-                load_operands_async<Q>(p, sm, 1, si.sbase + tri_index(nt, I, K1), si.sbase + tri_index(nt, K1, J));
-                cp_async_wait<1>();
-            } else {
-                cp_async_wait<0>();
-            }
-            __syncthreads();
-            if (pact) product_accumulate<Q>(sm, 0, acc, jj, rb);
-            if (K1 != K0) {
-                cp_async_wait<0>();
-                __syncthreads();
-                if (pact) product_accumulate<Q>(sm, 1, acc, jj, rb);
-            }
-            if (pact) {
-#pragma unroll
-                for (int rr = 0; rr < C::RPT; ++rr) {
-                    int16_t *cell = sm.val + (rb * C::RPT + rr) * C::VP + jj + 1;
-                    *cell = (int16_t)max((int)*cell, (int)(acc[rr] >> C::SH));
-                }
-            }
-            __syncthreads();
-        }
-        if (tr && tid == 0) tr[3] = global_timer_ns();
-        if (warp < 8) qcol_closure<Q, false>(sm, warp, lane, parity, (tr && warp == 7) ? tr + 7 : nullptr);
-        __syncthreads();
-    }
-    if (tr && tid == 0) tr[4] = global_timer_ns();
-
-    // ---- publish: row panel, column panel, edges (step a6 output), optional table block, score ----
-    {
-        uint8_t *rec = const_cast<uint8_t *>(rec_ptr<Q>(p, sidx));
-        uint32_t *ph = reinterpret_cast<uint32_t *>(rec);
+        if (tr && tid == 0) tr[4] = global_timer_ns();
+        // publish the whole record at once
+        uint32_t *ph = reinterpret_cast<uint32_t *>(cc.recX);
         uint32_t *pv = ph + C::PANEL_WORDS;
-        uint16_t *edge = reinterpret_cast<uint16_t *>(rec + 2 * C::PANEL_WORDS * 4);
+        uint16_t *edge = reinterpret_cast<uint16_t *>(cc.recX + 2 * C::PANEL_WORDS * 4);
         for (int e = tid; e < C::PANEL_WORDS; e += C::NTHR) {
             const int g = e / T, k = e % T;
             __stcg(ph + e, sm.Wst[(8 + g) * C::TP + k]);
@@ -752,6 +871,67 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             __stcg(edge + tid, (uint16_t)sm.val[tid + 1]);                       // top row  M(I*T, c)
             __stcg(edge + T + tid, (uint16_t)sm.val[tid * C::VP + T]);           // right column M(r, J*T+T-1)
         }
+    } else {
+        const int s_left = si.sbase + tri_index(nt, I, J - 1);
+        const int s_below = si.sbase + tri_index(nt, I + 1, J);
+        const int s_ii = si.sbase + tri_index(nt, I, I);
+        const int s_jj = si.sbase + tri_index(nt, J, J);
+        const int s_i1 = si.sbase + tri_index(nt, I, I + 1);
+        const int s_j1 = si.sbase + tri_index(nt, J - 1, J);
+        const int S = nstages(dp, p.delta);
+        cc.recZ = rec_ptr<Q>(p, s_left); cc.recY = rec_ptr<Q>(p, s_below);
+        cc.rowprogZ = p.rowprog + s_left; cc.colprogY = p.colprog + s_below;
+        if (dp >= 2) {
+            const int s_c = si.sbase + tri_index(nt, I + 1, J - 1);
+            cc.recC = rec_ptr<Q>(p, s_c); cc.doneC = p.done + s_c;
+        }
+        if (tid == 0) {
+            wait_flag_ge(p.done + s_ii, 1);
+            wait_flag_ge(p.done + s_jj, 1);
+            if (dp >= 3) { wait_flag_ge(p.done + s_i1, 1); wait_flag_ge(p.done + s_j1, 1); }
+            if (S > 0) wait_flag_ge(p.accstage + sidx, S);
+            if (tr) tr[1] = global_timer_ns();
+        }
+        __syncthreads();
+        // static words: row words of (I,I) -> Wst[0..7], column words of (J,J) -> Xst[8..15]; the tile's own
+        // words are not known yet: zero (= a valid lower bound)
+        {
+            const uint32_t *ph = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_ii));
+            const uint32_t *pv = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_jj)) + C::PANEL_WORDS;
+            for (int e = tid; e < C::PANEL_WORDS; e += C::NTHR) {
+                const int g = e / T, k = e % T;
+                sm.Wst[g * C::TP + k] = __ldcg(ph + e);
+                sm.Xst[(8 + g) * C::TP + k] = __ldcg(pv + e);
+            }
+            for (int e = tid; e < 8 * C::TP; e += C::NTHR) { sm.Wst[8 * C::TP + e] = 0; sm.Xst[e] = 0; }
+            if (dp >= 3) {
+                // static operands of the late products: row panel of (I,I+1), column panel of (J-1,J)
+                const uint32_t *ph1 = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_i1));
+                const uint32_t *pv1 = reinterpret_cast<const uint32_t *>(rec_ptr<Q>(p, s_j1)) + C::PANEL_WORDS;
+                uint32_t *WI1 = panel_WI1<Q>(sm), *XJ1 = panel_XJ1<Q>(sm);
+                for (int e = tid; e < C::PANEL_WORDS; e += C::NTHR) { WI1[e] = __ldcg(ph1 + e); XJ1[e] = __ldcg(pv1 + e); }
+            }
+        }
+        // bulk maxima gathered by the PROD stages (or zero)
+        if (S > 0) {
+            const int16_t *accg = p.acc + (size_t)sidx * T * T;
+            for (int e = tid; e < T * T; e += C::NTHR) sm.val[(e / T) * C::VP + (e % T) + 1] = __ldcg(accg + e);
+        } else {
+            for (int e = tid; e < T * T; e += C::NTHR) sm.val[(e / T) * C::VP + (e % T) + 1] = 0;
+        }
+        __syncthreads();
+        if (tr && tid == 0) tr[2] = tr[3] = global_timer_ns();
+        if (warp < 8) qcol_closure<Q, false>(sm, cc, warp, lane, (tr && warp == 7) ? tr + 7 : nullptr);
+        else if (warp == 8) close_row_loader<Q>(sm, cc, lane);
+        else if (warp == 9) close_publisher<Q>(sm, cc, lane);
+        else if (warp == 10) close_row_late<Q>(sm, cc, lane);
+        else if (warp == 11) close_col_late<Q>(sm, cc, lane);
+        __syncthreads();
+        if (tr && tid == 0) tr[4] = global_timer_ns();
+    }
+
+    // ---- optional table block, score, completion flags (step a8) ----
+    {
         const int n = si.n;
         if (p.table_out) {
             // out[(i-1)*n + (j-1)] = D(i,j) = M(i-1, j): r = i-1 <= n-1, 1 <= c <= n, c >= r+1
@@ -769,7 +949,12 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
         __threadfence();
         __syncthreads();
-        if (tid == 0) { st_release_gpu(p.done + sidx, 1); sm.misc[1] += 1; if (tr) tr[5] = global_timer_ns(); }
+        if (tid == 0) {
+            if (dp == 0) { st_release_gpu(cc.rowprogX, 8); st_release_gpu(cc.colprogX, 8); }
+            st_release_gpu(p.done + sidx, 1);
+            sm.misc[1] += 1;
+            if (tr) tr[5] = global_timer_ns();
+        }
     }
 }
 
@@ -788,7 +973,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR) fill_kernel(Params p)
         for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
         if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
     }
-    if (tid < 64) mbar_init(sm.mbar + tid, 1);
+    if (tid < C::MB_COUNT) mbar_init(sm.mbar + tid, 1);
     if (tid == 0) sm.misc[1] = 0;
     __syncthreads();
     const int total = p.hdr->total;
@@ -831,7 +1016,7 @@ static inline HostPlan host_plan(int T, int delta, const int32_t *lens, int coun
 
 struct WsLayout {
     size_t zero_bytes;   // prefix that must be zeroed before every fold
-    size_t off_hdr, off_stepC, off_stepP, off_curC, off_curP, off_done, off_accstage;
+    size_t off_hdr, off_stepC, off_stepP, off_curC, off_curP, off_done, off_accstage, off_rowprog, off_colprog;
     size_t off_seqinfo, off_tasks, off_codes, off_recs, off_acc, total;
 };
 
@@ -846,6 +1031,8 @@ static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int co
     w.off_curP = off; off += align_up((size_t)h.max_nt * 4, 256);
     w.off_done = off; off += align_up(h.tiles * 4, 256);
     w.off_accstage = off; off += align_up(h.tiles * 4, 256);
+    w.off_rowprog = off; off += align_up(h.tiles * 4, 256);
+    w.off_colprog = off; off += align_up(h.tiles * 4, 256);
     w.zero_bytes = off;
     w.off_seqinfo = off; off += align_up((size_t)count * sizeof(SeqInfo), 256);
     w.off_tasks = off; off += align_up(h.tasks * sizeof(int4), 256);
@@ -878,6 +1065,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     p.stepC = (int *)(base + w.off_stepC); p.stepP = (int *)(base + w.off_stepP);
     p.curC = (int *)(base + w.off_curC); p.curP = (int *)(base + w.off_curP);
     p.done = (int *)(base + w.off_done); p.accstage = (int *)(base + w.off_accstage);
+    p.rowprog = (int *)(base + w.off_rowprog); p.colprog = (int *)(base + w.off_colprog);
     p.seqinfo = (SeqInfo *)(base + w.off_seqinfo);
     p.tasks = (int4 *)(base + w.off_tasks);
     p.codes = (int8_t *)(base + w.off_codes);
