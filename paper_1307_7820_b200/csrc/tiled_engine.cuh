@@ -66,12 +66,20 @@ struct Cfg {
     static constexpr int STG_BYTES = 2 * 2 * PANEL_WORDS * 4;
     static constexpr int VP2 = T + 2;          // pitch of val2 (int16): odd word stride, a column of it is conflict-free
     static constexpr int VAL2_BYTES = (T * VP2 * 2 + 15) / 16 * 16;   // late products of block I+1 (kept apart: two warps merge concurrently)
-    // mbarriers (each completes once per closure): [0,64) q-tile (A,B) done, at B*8+A; [64,72) rows of q-row A
-    // of the left tile loaded; [72,80) columns of q-column B of the tile below loaded; [80,88) late products of
-    // q-row A merged; [88,96) late products of q-column B merged
-    static constexpr int MB_ROW = 64, MB_COL = 72, MB_RLATE = 80, MB_CLATE = 88, MB_COUNT = 96;
+    // closure warps: a warp runs G q-tiles of one anti-diagonal side by side (Q lanes each); NWV such warps cover
+    // the <= 8 q-tiles of a macro-step; NMH helper warps prepare the next macro-step's older complete groups
+    static constexpr int G = (32 / Q < 4) ? 32 / Q : 4;
+    static constexpr int NWV = (8 + G - 1) / G;
+    static constexpr int NMH = 2;
+    static constexpr int NROLE = NWV + NMH + 5;          // + row loader, column loader, publisher, row-late, column-late
+    static constexpr int STEP_THREADS = (NWV + NMH) * 32;   // participants of the per-macro-step named barrier
+    // mbarriers (each completes once per closure): [0,15) macro-step u done; [16,24) rows of q-row A of the left
+    // tile loaded; [24,32) columns of q-column B of the tile below loaded; [32,40) late products of q-row A merged;
+    // [40,48) late products of q-column B merged
+    static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_RLATE = 32, MB_CLATE = 40, MB_COUNT = 48;
     static constexpr int MBAR_BYTES = MB_COUNT * 8;
-    static constexpr int POST_BYTES = VAL_BYTES + VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
+    static_assert(NROLE * 32 <= NTHR, "closure roles must fit the CTA");
+    static constexpr int POST_BYTES = VAL_BYTES + 2 * VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
     // dynamic shared memory needed when the dynamic window starts at shared address `base`
     static constexpr size_t smem_bytes_for(size_t base)
     {
@@ -239,6 +247,7 @@ struct Smem {
     int16_t *valraw;     // start of the value array including its guard rows
     int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
     int16_t *val2;       // [T][VP2] late products of block K = I+1 (written by the column-late helper, merged by the closure warps)
+    int16_t *val3;       // [T][VP2] older complete groups of the closure (written by the mini helpers one macro-step ahead)
     uint32_t *stg;       // [2][2][PANEL_WORDS] product operands, double buffered: [buf][0]=PH, [buf][1]=PV
     int8_t *codeR;       // [T] codes of the rows
     int8_t *codeC;       // [T] codes of the columns
@@ -257,6 +266,7 @@ struct Smem {
         tbl = p; tbl_sa = tsa; p += (C::TBL_BYTES + 15) / 16 * 16;
         valraw = (int16_t *)p; val = valraw + Q * C::VP; p += C::VAL_BYTES;     // val[0] = row 0; Q guard rows on either side
         val2 = (int16_t *)p; p += C::VAL2_BYTES;
+        val3 = (int16_t *)p; p += C::VAL2_BYTES;
         stg = (uint32_t *)p; p += C::STG_BYTES;
         codeR = (int8_t *)p; p += C::T;
         codeC = (int8_t *)p; p += C::T;
@@ -494,7 +504,7 @@ __device__ __forceinline__ uint32_t lookup_tagged(const Smem<Q> &sm, uint32_t S)
 // closure (W = Wst, X = Xst) and for the late products (operand panels of the neighbouring blocks).
 template <int Q>
 __device__ __forceinline__ void qtile_groups(const Smem<Q> &sm, int A, int B, const uint32_t *W, int wp, const uint32_t *X, int xp,
-                                             int zlo, int zhi, int lane, bool merge2 = false)
+                                             int zlo, int zhi, int lane, bool merge2 = false, bool out3 = false)
 {
     using C = Cfg<Q>;
     constexpr int VP = C::VP, SH = C::SH;
@@ -520,7 +530,9 @@ __device__ __forceinline__ void qtile_groups(const Smem<Q> &sm, int A, int B, co
 #pragma unroll
     for (int i = 0; i < NX; ++i) {
         const int x = xr + i * RS;
-        if (x < Q) {
+        if (x < Q && out3) {
+            sm.val3[(abot - x) * C::VP2 + mc] = (int16_t)(best[i] >> SH);        // written once per cell
+        } else if (x < Q) {
             int16_t *cell = sm.val + (abot - x) * VP + mc + 1;
             int v = max((int)*cell, (int)(best[i] >> SH));
             if (merge2) v = max(v, (int)sm.val2[(abot - x) * C::VP2 + mc]);      // late products of block I+1
@@ -532,14 +544,13 @@ __device__ __forceinline__ void qtile_groups(const Smem<Q> &sm, int A, int B, co
 // (C) phase of q-tile (A,B): 2Q unrolled skewed steps; every address is lane base + immediate.
 // MERGED: q-tile (B,B) of a diagonal super-tile (head and tail are one lookup; c-a = s-Q+1 for every lane).
 template <int Q, bool DIAG, bool MERGED>
-__device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int lane)
+__device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int lane, bool own)
 {
     using C = Cfg<Q>;
     constexpr int TP = C::TP, VP = C::VP, SH = C::SH, HB = C::HB;
     constexpr uint32_t FULL = 0xffffffffu;
     constexpr int ZOFF = DIAG ? 0 : 8;
-    const int y = lane % Q;                              // lanes >= Q shadow lane y and store nothing
-    const bool own = lane < Q;
+    const int y = lane % Q;                              // lane group lane/Q runs q-tile (A,B); !own: shadow, stores nothing
     const bool firstcol = (y == 0), lastcol = (y == Q - 1);
     const int src1 = firstcol ? lane : lane - 1, src2 = (y >= 2) ? lane - 2 : lane;
     const uint32_t w2mask = (y >= 2) ? FULL : 0u;
@@ -620,6 +631,7 @@ struct CloseCtx {
     uint8_t *recX;       // record of this tile
     const int *rowprogZ, *colprogY, *doneC;
     int *rowprogX, *colprogX;
+    unsigned long long *prof; // trace record of this closure, or NULL
     unsigned long long *ev;   // fine trace of this closure (RNA4R_TRACE_WORDS > 8), else NULL
 };
 #define RNA4R_EV(cc, idx) do { if (RNA4R_TRACE_WORDS > 8 && (cc).ev && lane == 0) (cc).ev[idx] = global_timer_ns(); } while (0)
@@ -630,64 +642,144 @@ __device__ __forceinline__ void warp_wait_flag_ge(const int *flag, int v, int la
     __syncwarp();
 }
 
-// closure warp B (q-tile column B), off-diagonal super-tile and diagonal super-tile
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// q-tile t of macro-step u (anti-diagonal (7-A)+B = u), counted from the bottom-left
+__device__ __forceinline__ void qtile_of(int u, int t, int &A, int &B)
+{
+    const int Amax = min(7, 14 - u);
+    A = Amax - t;
+    B = u - (7 - A);
+}
+__device__ __forceinline__ int qtile_count(int u) { return min(7, 14 - u) - max(0, 7 - u) + 1; }
+
+// Before its cell wavefront a lane group folds into val[][] everything that is known about its q-tile:
+// the late products of block I+1 (val2), the older complete groups prepared by the mini helpers (val3) and
+// the two complete groups that were only finished in the previous macro-step -- the lowest and the highest z
+// of the q-tile's range [A+1, ZOFF+B-1] (column word of the q-tile below, row word of the q-tile to the left).
 template <int Q, bool DIAG>
-__device__ __forceinline__ void qcol_closure(const Smem<Q> &sm, const CloseCtx &cc, int B, int lane, unsigned long long *prof = nullptr)
+__device__ __forceinline__ void qtile_fresh_merge(const Smem<Q> &sm, int A, int B, int lane, bool own, bool use2)
 {
     using C = Cfg<Q>;
-    constexpr int T = C::T, TP = C::TP, VP = C::VP;
-    long long t_poll = 0, t_mini = 0, t_wave = 0, t0 = 0;
+    constexpr int TP = C::TP, VP = C::VP, VP2 = C::VP2, SH = C::SH;
     constexpr int ZOFF = DIAG ? 0 : 8;
-    const int Astart = DIAG ? B : 7;
-    if (DIAG) {
-        if (lane == 0) for (int A = B + 1; A < 8; ++A) mbar_arrive(sm.mbar + B * 8 + A);      // q-tiles below the diagonal: nothing to do
-    } else {
-        // ---- my columns of the tile below: column words (late products) and its top row (my bottom edge)
+    const int y = lane % Q;
+    const int c = B * Q + y;
+    const int abot = A * Q + Q - 1;
+    const int lo = A + 1, hi = ZOFF + B - 1;
+    const bool has1 = lo <= hi, has2 = hi > lo;
+    const uint32_t X1 = has1 ? sm.Xst[lo * TP + c] : 0u;
+    const uint32_t X2 = has2 ? sm.Xst[hi * TP + c] : 0u;
+    const uint32_t *w1 = sm.Wst + (has1 ? lo : 0) * TP + abot;
+    const uint32_t *w2 = sm.Wst + (has2 ? hi : 0) * TP + abot;
+    const uint32_t m1 = has1 ? 0xffffffffu : 0u, m2 = has2 ? 0xffffffffu : 0u;
+#pragma unroll
+    for (int x = 0; x < Q; ++x) {
+        const int a = abot - x;
+        int v = max((int)sm.val[a * VP + c + 1], (int)sm.val3[a * VP2 + c]);
+        if (use2) v = max(v, (int)sm.val2[a * VP2 + c]);
+        const uint32_t b1 = lookup_tagged<Q>(sm, (w1[-x] & m1) + X1);     // a zero pair looks up R[0][0] = 0
+        const uint32_t b2 = lookup_tagged<Q>(sm, (w2[-x] & m2) + X2);
+        v = max(v, (int)(max(b1, b2) >> SH));
+        if (own) sm.val[a * VP + c + 1] = (int16_t)v;
+    }
+}
+
+// closure warp w of NWV: G q-tiles of the current anti-diagonal side by side, macro-step by macro-step
+template <int Q, bool DIAG>
+__device__ __forceinline__ void close_wave(const Smem<Q> &sm, const CloseCtx &cc, int w, int lane)
+{
+    using C = Cfg<Q>;
+    const int j = lane / Q;
+    long long pf_merge = 0, pf_wave = 0, pf_bar = 0;
+    named_bar_sync(1, C::STEP_THREADS);                 // val3 is cleared
+#pragma unroll 1
+    for (int u = DIAG ? 7 : 0; u < 15; ++u) {
+        if (!DIAG && u <= 7) {
+            mbar_wait(sm.mbar + C::MB_RLATE + 7 - u, cc.parity);      // left edge and late products of the q-row that starts now
+            mbar_wait(sm.mbar + C::MB_CLATE + u, cc.parity);          // bottom edge and late products of the q-column that starts now
+        }
+        const int cnt = qtile_count(u);
+        const int t = w * C::G + j;
+        const bool own = (j < C::G) && (t < cnt);
+        int A, B;
+        qtile_of(u, own ? t : 0, A, B);
+        const long long c0 = clock64();
+        qtile_fresh_merge<Q, DIAG>(sm, A, B, lane, own, !DIAG && cc.dp >= 3);
+        __syncwarp();
+        const long long c1 = clock64();
+        if (DIAG && u == 7) qtile_wave<Q, true, true>(sm, A, B, lane, own);
+        else qtile_wave<Q, DIAG, false>(sm, A, B, lane, own);
+        const long long c2 = clock64();
+        named_bar_sync(1, C::STEP_THREADS);
+        const long long c3 = clock64();
+        pf_merge += c1 - c0; pf_wave += c2 - c1; pf_bar += c3 - c2;
+        if (w == 0 && lane == 0) mbar_arrive(sm.mbar + C::MB_STEP + u);
+        if (w == 0) RNA4R_EV(cc, 8 + u);
+    }
+    if (cc.prof && w == 0 && lane == 0)
+        cc.prof[7] = ((unsigned long long)(pf_merge & 0x1fffff)) | ((unsigned long long)(pf_wave & 0x1fffff) << 21) | ((unsigned long long)(pf_bar & 0x1fffff) << 42);
+}
+
+// mini helper h of NMH: while the closure warps run macro-step u, the older complete groups
+// z in [A+2, ZOFF+B-2] of the q-tiles of macro-step u+1 (all finished by macro-step u-1) -> val3
+template <int Q, bool DIAG>
+__device__ __forceinline__ void close_mini_helper(const Smem<Q> &sm, const CloseCtx &cc, int h, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr int ZOFF = DIAG ? 0 : 8;
+    {
+        uint32_t *z = reinterpret_cast<uint32_t *>(sm.val3);
+        for (int e = h * 32 + lane; e < C::VAL2_BYTES / 4; e += C::NMH * 32) z[e] = 0;
+    }
+    named_bar_sync(1, C::STEP_THREADS);
+#pragma unroll 1
+    for (int u = DIAG ? 7 : 0; u < 15; ++u) {
+        if (u + 1 < 15) {
+            const int cnt = qtile_count(u + 1);
+            for (int t = h; t < cnt; t += C::NMH) {
+                int A, B;
+                qtile_of(u + 1, t, A, B);
+                qtile_groups<Q>(sm, A, B, sm.Wst, C::TP, sm.Xst, C::TP, A + 2, ZOFF + B - 2, lane, false, true);
+            }
+        }
+        named_bar_sync(1, C::STEP_THREADS);
+    }
+}
+
+// helper warp: columns of the tile below, q-column by q-column as it publishes them (column words for the
+// late products, top-row values = my bottom edge), and the corner value
+template <int Q>
+__device__ __forceinline__ void close_col_loader(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T, VP = C::VP;
+    const uint32_t *pv = reinterpret_cast<const uint32_t *>(cc.recY) + C::PANEL_WORDS;
+    const uint16_t *etop = reinterpret_cast<const uint16_t *>(cc.recY + 2 * C::PANEL_WORDS * 4);
+    uint32_t *YX = panel_YX<Q>(sm);
+    if (lane == 0) {
+        // corner M((I+1)T, JT-1) = top row of (I+1,J-1) at its last column
+        int corner = 0;
+        if (cc.recC) {
+            while (ld_acquire_gpu(cc.doneC) < 1) __nanosleep(40);
+            corner = __ldcg(reinterpret_cast<const uint16_t *>(cc.recC + 2 * C::PANEL_WORDS * 4) + T - 1);
+        }
+        sm.val[T * VP] = (int16_t)corner;
+    }
+    for (int B = 0; B < 8; ++B) {
         warp_wait_flag_ge(cc.colprogY, B + 1, lane);
-        const uint32_t *pv = reinterpret_cast<const uint32_t *>(cc.recY) + C::PANEL_WORDS;
-        const uint16_t *etop = reinterpret_cast<const uint16_t *>(cc.recY + 2 * C::PANEL_WORDS * 4);
-        uint32_t *YX = panel_YX<Q>(sm);
         for (int e = lane; e < 8 * Q; e += 32) {
             const int g = e / Q, k = B * Q + e % Q;
             YX[g * T + k] = __ldcg(pv + g * T + k);
         }
         if (lane < Q) sm.val[T * VP + B * Q + lane + 1] = (int16_t)__ldcg(etop + B * Q + lane);
-        if (B == 0 && lane == 0) {
-            // corner M((I+1)T, JT-1) = top row of (I+1,J-1) at its last column
-            int corner = 0;
-            if (cc.recC) {
-                while (ld_acquire_gpu(cc.doneC) < 1) __nanosleep(40);
-                corner = __ldcg(reinterpret_cast<const uint16_t *>(cc.recC + 2 * C::PANEL_WORDS * 4) + T - 1);
-            }
-            sm.val[T * VP] = (int16_t)corner;
-        }
         __syncwarp();
         if (lane == 0) mbar_arrive(sm.mbar + C::MB_COL + B);
         RNA4R_EV(cc, 144 + B);
-        mbar_wait(sm.mbar + C::MB_CLATE + B, cc.parity);        // late products of my columns
     }
-#pragma unroll 1
-    for (int A = Astart; A >= 0; --A) {
-        if (prof) t0 = clock64();
-        // ---- wait for q-tile (A, B-1) and for the late products (and edges) of (A, B)
-        if (B > 0) mbar_wait(sm.mbar + (B - 1) * 8 + A, cc.parity);
-        if (!DIAG) mbar_wait(sm.mbar + C::MB_RLATE + A, cc.parity);   // left edge and late products of q-row A
-        __syncwarp();
-        RNA4R_EV(cc, 72 + B * 8 + A);
-        if (prof) { const long long t1 = clock64(); t_poll += t1 - t0; t0 = t1; }
-        qtile_groups<Q>(sm, A, B, sm.Wst, TP, sm.Xst, TP, A + 1, ZOFF + B - 1, lane, !DIAG && cc.dp >= 3);
-        __syncwarp();
-        if (prof) { const long long t1 = clock64(); t_mini += t1 - t0; t0 = t1; }
-        if (DIAG && A == B) qtile_wave<Q, true, true>(sm, A, B, lane);
-        else qtile_wave<Q, DIAG, false>(sm, A, B, lane);
-        // ---- hand the q-tile to warp B+1 (and to the publisher)
-        __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + B * 8 + A);
-        RNA4R_EV(cc, 8 + B * 8 + A);
-        if (prof) { const long long t1 = clock64(); t_wave += t1 - t0; t0 = t1; }
-    }
-    if (prof && lane == 0)
-        prof[0] = ((unsigned long long)(t_poll & 0x1fffff)) | ((unsigned long long)(t_mini & 0x1fffff) << 21) | ((unsigned long long)(t_wave & 0x1fffff) << 42);
 }
 
 // helper warp: rows of the left tile, q-row by q-row as it publishes them (row words for the late
@@ -725,9 +817,9 @@ __device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCt
     uint32_t *pv = ph + C::PANEL_WORDS;
     uint16_t *edge = reinterpret_cast<uint16_t *>(cc.recX + 2 * C::PANEL_WORDS * 4);
     for (int i = 0; i < 8; ++i) {
+        mbar_wait(sm.mbar + C::MB_STEP + 7 + i, cc.parity);      // q-tiles (0,i) and (7-i,7) are on anti-diagonal 7+i
         {
             const int B = i;
-            mbar_wait(sm.mbar + B * 8 + 0, cc.parity);
             for (int e = lane; e < 8 * Q; e += 32) {
                 const int g = e / Q, k = B * Q + e % Q;
                 __stcg(pv + g * T + k, sm.Xst[g * TP + k]);
@@ -740,7 +832,6 @@ __device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCt
         }
         {
             const int A = 7 - i;
-            mbar_wait(sm.mbar + 7 * 8 + A, cc.parity);
             for (int e = lane; e < 8 * Q; e += 32) {
                 const int g = e / Q, k = A * Q + e % Q;
                 __stcg(ph + g * T + k, sm.Wst[(8 + g) * TP + k]);
@@ -845,6 +936,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
     cc.parity = (uint32_t)sm.misc[1] & 1u;    // closures this CTA has run so far: phase of its mbarriers
     cc.recX = const_cast<uint8_t *>(rec_ptr<Q>(p, sidx));
     cc.rowprogX = p.rowprog + sidx; cc.colprogX = p.colprog + sidx;
+    cc.prof = tr;
     cc.ev = (RNA4R_TRACE_WORDS > 8) ? tr : nullptr;
     cc.recZ = cc.recY = cc.recC = nullptr; cc.rowprogZ = cc.colprogY = cc.doneC = nullptr;
 
@@ -853,9 +945,13 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         for (int e = tid; e < C::VAL_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(sm.valraw)[e] = 0;
         for (int e = tid; e < C::WROWS * C::TP; e += C::NTHR) { sm.Wst[e] = 0; sm.Xst[e] = 0; }
         __syncthreads();
-        if (warp < 8) qcol_closure<Q, true>(sm, cc, warp, lane, (tr && warp == 7) ? tr + 7 : nullptr);
-        else if (warp == 8)
-            for (int e = lane; e < C::MB_COUNT - C::MB_ROW; e += 32) mbar_arrive(sm.mbar + C::MB_ROW + e);   // keep the phases in step
+        if (warp < C::NWV) close_wave<Q, true>(sm, cc, warp, lane);
+        else if (warp < C::NWV + C::NMH) close_mini_helper<Q, true>(sm, cc, warp - C::NWV, lane);
+        else if (warp == C::NWV + C::NMH) {
+            // keep the phases of the barriers a diagonal super-tile does not use in step
+            for (int e = lane; e < C::MB_COUNT - C::MB_ROW; e += 32) mbar_arrive(sm.mbar + C::MB_ROW + e);
+            if (lane < 7) mbar_arrive(sm.mbar + C::MB_STEP + lane);
+        }
         __syncthreads();
         if (tr && tid == 0) tr[4] = global_timer_ns();
         // publish the whole record at once
@@ -921,11 +1017,13 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         }
         __syncthreads();
         if (tr && tid == 0) tr[2] = tr[3] = global_timer_ns();
-        if (warp < 8) qcol_closure<Q, false>(sm, cc, warp, lane, (tr && warp == 7) ? tr + 7 : nullptr);
-        else if (warp == 8) close_row_loader<Q>(sm, cc, lane);
-        else if (warp == 9) close_publisher<Q>(sm, cc, lane);
-        else if (warp == 10) close_row_late<Q>(sm, cc, lane);
-        else if (warp == 11) close_col_late<Q>(sm, cc, lane);
+        if (warp < C::NWV) close_wave<Q, false>(sm, cc, warp, lane);
+        else if (warp < C::NWV + C::NMH) close_mini_helper<Q, false>(sm, cc, warp - C::NWV, lane);
+        else if (warp == C::NWV + C::NMH) close_row_loader<Q>(sm, cc, lane);
+        else if (warp == C::NWV + C::NMH + 1) close_col_loader<Q>(sm, cc, lane);
+        else if (warp == C::NWV + C::NMH + 2) close_publisher<Q>(sm, cc, lane);
+        else if (warp == C::NWV + C::NMH + 3) close_row_late<Q>(sm, cc, lane);
+        else if (warp == C::NWV + C::NMH + 4) close_col_late<Q>(sm, cc, lane);
         __syncthreads();
         if (tr && tid == 0) tr[4] = global_timer_ns();
     }
