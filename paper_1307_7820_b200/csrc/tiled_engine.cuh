@@ -48,7 +48,7 @@ struct Cfg {
     static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
     static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
     static constexpr int NTHR = WTHR + 128;    // + 4 helper warps of the closure: loader, publisher, 2 x late products
-    static constexpr int HW0 = WTHR / 32;      // first helper warp
+    static constexpr int MIN_CTAS = (Q <= 8) ? 3 : 1;   // register budget: 3 CTAs per SM while the table is small
     static constexpr int RPT = 2 * Q;          // rows per thread in the product phase
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
     static constexpr int VP = T + 1;           // pitch of the value array (int16): a wavefront step is conflict-free
@@ -71,12 +71,13 @@ struct Cfg {
     static constexpr int G = (32 / Q < 4) ? 32 / Q : 4;
     static constexpr int NWV = (8 + G - 1) / G;
     static constexpr int NMH = 2;
-    static constexpr int NROLE = NWV + NMH + 5;          // + row loader, column loader, publisher, row-late, column-late
+    static constexpr int NROLE = NWV + NMH + 8;          // + row/column loader, row/column publisher, 2 row-late, 2 column-late
     static constexpr int STEP_THREADS = (NWV + NMH) * 32;   // participants of the per-macro-step named barrier
     // mbarriers (each completes once per closure): [0,15) macro-step u done; [16,24) rows of q-row A of the left
-    // tile loaded; [24,32) columns of q-column B of the tile below loaded; [32,40) late products of q-row A merged;
-    // [40,48) late products of q-column B merged
-    static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_RLATE = 32, MB_CLATE = 40, MB_COUNT = 48;
+    // tile loaded; [24,32) columns of q-column B of the tile below loaded; [32,48) late products of q-row A merged
+    // for the left / right half of the columns (32+A, 40+A); [48,64) late products of q-column B merged for the
+    // upper / lower half of the rows (48+B, 56+B)
+    static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_RLATE = 32, MB_CLATE = 48, MB_COUNT = 64;
     static constexpr int MBAR_BYTES = MB_COUNT * 8;
     static_assert(NROLE * 32 <= NTHR, "closure roles must fit the CTA");
     static constexpr int POST_BYTES = VAL_BYTES + 2 * VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
@@ -656,39 +657,78 @@ __device__ __forceinline__ void qtile_of(int u, int t, int &A, int &B)
 }
 __device__ __forceinline__ int qtile_count(int u) { return min(7, 14 - u) - max(0, 7 - u) + 1; }
 
-// Before its cell wavefront a lane group folds into val[][] everything that is known about its q-tile:
-// the late products of block I+1 (val2), the older complete groups prepared by the mini helpers (val3) and
-// the two complete groups that were only finished in the previous macro-step -- the lowest and the highest z
-// of the q-tile's range [A+1, ZOFF+B-1] (column word of the q-tile below, row word of the q-tile to the left).
+// Before the cell wavefronts of a macro-step, everything that is known about its q-tiles is folded into val[][]:
+// the late products of block I+1 (val2), the older complete groups prepared by the mini helpers (val3) and the
+// two complete groups that were only finished in the previous macro-step -- the lowest and the highest z of the
+// q-tile's range [A+1, ZOFF+B-1] (column word of the q-tile below, row word of the q-tile to the left).
+// One warp per q-tile, all 32 lanes (the closure warps and the mini helpers share the q-tiles of the macro-step).
 template <int Q, bool DIAG>
-__device__ __forceinline__ void qtile_fresh_merge(const Smem<Q> &sm, int A, int B, int lane, bool own, bool use2)
+__device__ __forceinline__ void qtile_fresh_merge(const Smem<Q> &sm, int A, int B, int lane, bool use2)
 {
     using C = Cfg<Q>;
     constexpr int TP = C::TP, VP = C::VP, VP2 = C::VP2, SH = C::SH;
     constexpr int ZOFF = DIAG ? 0 : 8;
-    const int y = lane % Q;
-    const int c = B * Q + y;
+    constexpr int RS = (32 / Q > Q) ? Q : 32 / Q;        // row slots
+    constexpr int NX = (Q + RS - 1) / RS;                // rows per lane
+    const int my = lane % Q, xr = lane / Q;
+    if (xr >= RS) return;
+    const int c = B * Q + my;
     const int abot = A * Q + Q - 1;
     const int lo = A + 1, hi = ZOFF + B - 1;
     const bool has1 = lo <= hi, has2 = hi > lo;
     const uint32_t X1 = has1 ? sm.Xst[lo * TP + c] : 0u;
     const uint32_t X2 = has2 ? sm.Xst[hi * TP + c] : 0u;
-    const uint32_t *w1 = sm.Wst + (has1 ? lo : 0) * TP + abot;
-    const uint32_t *w2 = sm.Wst + (has2 ? hi : 0) * TP + abot;
+    const uint32_t *w1 = sm.Wst + (has1 ? lo : 0) * TP;
+    const uint32_t *w2 = sm.Wst + (has2 ? hi : 0) * TP;
     const uint32_t m1 = has1 ? 0xffffffffu : 0u, m2 = has2 ? 0xffffffffu : 0u;
 #pragma unroll
-    for (int x = 0; x < Q; ++x) {
-        const int a = abot - x;
-        int v = max((int)sm.val[a * VP + c + 1], (int)sm.val3[a * VP2 + c]);
-        if (use2) v = max(v, (int)sm.val2[a * VP2 + c]);
-        const uint32_t b1 = lookup_tagged<Q>(sm, (w1[-x] & m1) + X1);     // a zero pair looks up R[0][0] = 0
-        const uint32_t b2 = lookup_tagged<Q>(sm, (w2[-x] & m2) + X2);
-        v = max(v, (int)(max(b1, b2) >> SH));
-        if (own) sm.val[a * VP + c + 1] = (int16_t)v;
+    for (int i = 0; i < NX; ++i) {
+        const int x = xr + i * RS;
+        if (x < Q) {
+            const int a = abot - x;
+            int v = max((int)sm.val[a * VP + c + 1], (int)sm.val3[a * VP2 + c]);
+            if (use2) v = max(v, (int)sm.val2[a * VP2 + c]);
+            const uint32_t b1 = lookup_tagged<Q>(sm, (w1[a] & m1) + X1);     // a zero pair looks up R[0][0] = 0
+            const uint32_t b2 = lookup_tagged<Q>(sm, (w2[a] & m2) + X2);
+            v = max(v, (int)(max(b1, b2) >> SH));
+            sm.val[a * VP + c + 1] = (int16_t)v;
+        }
     }
 }
 
-// closure warp w of NWV: G q-tiles of the current anti-diagonal side by side, macro-step by macro-step
+// what macro-step u of an off-diagonal super-tile newly touches: q-row 7-u enters at column 0 (left half of
+// its late products, left edge), q-column u enters at row 7 (lower half, bottom edge); four macro-steps later
+// they reach the other half
+template <int Q>
+__device__ __forceinline__ void step_waits(const Smem<Q> &sm, const CloseCtx &cc, int u)
+{
+    using C = Cfg<Q>;
+    if (u <= 7) {
+        mbar_wait(sm.mbar + C::MB_RLATE + 7 - u, cc.parity);
+        mbar_wait(sm.mbar + C::MB_CLATE + 8 + u, cc.parity);
+    }
+    if (u >= 4 && u <= 11) {
+        mbar_wait(sm.mbar + C::MB_RLATE + 8 + 11 - u, cc.parity);
+        mbar_wait(sm.mbar + C::MB_CLATE + u - 4, cc.parity);
+    }
+}
+
+// phase F of macro-step u, step warp sw of NWV+NMH
+template <int Q, bool DIAG>
+__device__ __forceinline__ void macro_fresh(const Smem<Q> &sm, const CloseCtx &cc, int u, int sw, int lane)
+{
+    using C = Cfg<Q>;
+    const int cnt = qtile_count(u);
+    for (int t = sw; t < cnt; t += C::NWV + C::NMH) {
+        int A, B;
+        qtile_of(u, t, A, B);
+        qtile_fresh_merge<Q, DIAG>(sm, A, B, lane, !DIAG && cc.dp >= 3);
+    }
+}
+
+// closure warp w of NWV: G q-tiles of the current anti-diagonal side by side, macro-step by macro-step.
+// A macro-step is phase F (fresh merge, all step warps) | barrier | phase W (cell wavefronts here, older groups
+// of the next macro-step in the mini helpers) | barrier.
 template <int Q, bool DIAG>
 __device__ __forceinline__ void close_wave(const Smem<Q> &sm, const CloseCtx &cc, int w, int lane)
 {
@@ -698,21 +738,20 @@ __device__ __forceinline__ void close_wave(const Smem<Q> &sm, const CloseCtx &cc
     named_bar_sync(1, C::STEP_THREADS);                 // val3 is cleared
 #pragma unroll 1
     for (int u = DIAG ? 7 : 0; u < 15; ++u) {
-        if (!DIAG && u <= 7) {
-            mbar_wait(sm.mbar + C::MB_RLATE + 7 - u, cc.parity);      // left edge and late products of the q-row that starts now
-            mbar_wait(sm.mbar + C::MB_CLATE + u, cc.parity);          // bottom edge and late products of the q-column that starts now
-        }
+        const long long c0 = clock64();
+        if (!DIAG) step_waits<Q>(sm, cc, u);
+        macro_fresh<Q, DIAG>(sm, cc, u, w, lane);
+        named_bar_sync(1, C::STEP_THREADS);
+        const long long c1 = clock64();
         const int cnt = qtile_count(u);
         const int t = w * C::G + j;
         const bool own = (j < C::G) && (t < cnt);
         int A, B;
         qtile_of(u, own ? t : 0, A, B);
-        const long long c0 = clock64();
-        qtile_fresh_merge<Q, DIAG>(sm, A, B, lane, own, !DIAG && cc.dp >= 3);
-        __syncwarp();
-        const long long c1 = clock64();
-        if (DIAG && u == 7) qtile_wave<Q, true, true>(sm, A, B, lane, own);
-        else qtile_wave<Q, DIAG, false>(sm, A, B, lane, own);
+        if (w * C::G < cnt) {
+            if (DIAG && u == 7) qtile_wave<Q, true, true>(sm, A, B, lane, own);
+            else qtile_wave<Q, DIAG, false>(sm, A, B, lane, own);
+        }
         const long long c2 = clock64();
         named_bar_sync(1, C::STEP_THREADS);
         const long long c3 = clock64();
@@ -724,8 +763,9 @@ __device__ __forceinline__ void close_wave(const Smem<Q> &sm, const CloseCtx &cc
         cc.prof[7] = ((unsigned long long)(pf_merge & 0x1fffff)) | ((unsigned long long)(pf_wave & 0x1fffff) << 21) | ((unsigned long long)(pf_bar & 0x1fffff) << 42);
 }
 
-// mini helper h of NMH: while the closure warps run macro-step u, the older complete groups
-// z in [A+2, ZOFF+B-2] of the q-tiles of macro-step u+1 (all finished by macro-step u-1) -> val3
+// mini helper h of NMH: shares phase F; in phase W, while the closure warps run the cell wavefronts of
+// macro-step u, the older complete groups z in [A+2, ZOFF+B-2] of the q-tiles of macro-step u+1 (all finished
+// by macro-step u-1) -> val3
 template <int Q, bool DIAG>
 __device__ __forceinline__ void close_mini_helper(const Smem<Q> &sm, const CloseCtx &cc, int h, int lane)
 {
@@ -738,6 +778,9 @@ __device__ __forceinline__ void close_mini_helper(const Smem<Q> &sm, const Close
     named_bar_sync(1, C::STEP_THREADS);
 #pragma unroll 1
     for (int u = DIAG ? 7 : 0; u < 15; ++u) {
+        if (!DIAG) step_waits<Q>(sm, cc, u);
+        macro_fresh<Q, DIAG>(sm, cc, u, C::NWV + h, lane);
+        named_bar_sync(1, C::STEP_THREADS);
         if (u + 1 < 15) {
             const int cnt = qtile_count(u + 1);
             for (int t = h; t < cnt; t += C::NMH) {
@@ -805,11 +848,11 @@ __device__ __forceinline__ void close_row_loader(const Smem<Q> &sm, const CloseC
     }
 }
 
-// helper warp: publishes the tile q-row by q-row and q-column by q-column (step a6 output): row words and
-// right-column values of q-row A once q-tile (A,7) is done, column words and top-row values of q-column B
-// once q-tile (0,B) is done.
+// helper warps: publish the tile q-column by q-column (which = 0) and q-row by q-row (which = 1) (step a6
+// output): column words and top-row values of q-column B once q-tile (0,B) is done, row words and right-column
+// values of q-row A once q-tile (A,7) is done -- both are on anti-diagonal 7+i.
 template <int Q>
-__device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+__device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCtx &cc, int which, int lane)
 {
     using C = Cfg<Q>;
     constexpr int T = C::T, TP = C::TP, VP = C::VP;
@@ -817,27 +860,24 @@ __device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCt
     uint32_t *pv = ph + C::PANEL_WORDS;
     uint16_t *edge = reinterpret_cast<uint16_t *>(cc.recX + 2 * C::PANEL_WORDS * 4);
     for (int i = 0; i < 8; ++i) {
-        mbar_wait(sm.mbar + C::MB_STEP + 7 + i, cc.parity);      // q-tiles (0,i) and (7-i,7) are on anti-diagonal 7+i
-        {
+        mbar_wait(sm.mbar + C::MB_STEP + 7 + i, cc.parity);
+        if (which == 0) {
             const int B = i;
             for (int e = lane; e < 8 * Q; e += 32) {
                 const int g = e / Q, k = B * Q + e % Q;
                 __stcg(pv + g * T + k, sm.Xst[g * TP + k]);
             }
             if (lane < Q) __stcg(edge + B * Q + lane, (uint16_t)sm.val[B * Q + lane + 1]);           // top row  M(I*T, c)
-            __threadfence();
             __syncwarp();
             if (lane == 0) st_release_gpu(cc.colprogX, B + 1);
             RNA4R_EV(cc, 224 + B);
-        }
-        {
+        } else {
             const int A = 7 - i;
             for (int e = lane; e < 8 * Q; e += 32) {
                 const int g = e / Q, k = A * Q + e % Q;
                 __stcg(ph + g * T + k, sm.Wst[(8 + g) * TP + k]);
             }
             if (lane < Q) __stcg(edge + T + A * Q + lane, (uint16_t)sm.val[(A * Q + lane) * VP + T]);   // right column M(r, J*T+T-1)
-            __threadfence();
             __syncwarp();
             if (lane == 0) st_release_gpu(cc.rowprogX, 8 - A);
             RNA4R_EV(cc, 216 + A);
@@ -851,13 +891,13 @@ __device__ __forceinline__ void close_publisher(const Smem<Q> &sm, const CloseCt
 // over the 8 groups of the block; a lane owns one column (row) and NR rows (columns), so the words of the
 // short side are warp-uniform broadcast loads, as in the bulk product.
 template <int Q>
-__device__ __forceinline__ void late_strip(const Smem<Q> &sm, const uint32_t *U, int u0, const uint32_t *L, int16_t *out, int out_us, int out_ls,
-                                           bool domax, int lane)
+__device__ __forceinline__ void late_strip(const Smem<Q> &sm, const uint32_t *U, int u0, const uint32_t *L, int l0, int l1, int16_t *out,
+                                           int out_us, int out_ls, bool domax, int lane)
 {
-    // U[g*T + u0 + i], i < Q: the uniform side; L[g*T + l], l < T: the lane side; out[(u0+i)*out_us + l*out_ls]
+    // U[g*T + u0 + i], i < Q: the uniform side; L[g*T + l], l0 <= l < l1: the lane side; out[(u0+i)*out_us + l*out_ls]
     using C = Cfg<Q>;
     constexpr int T = C::T, SH = C::SH;
-    for (int l = lane; l < T; l += 32) {
+    for (int l = l0 + lane; l < l1; l += 32) {
         uint32_t acc[Q];
 #pragma unroll
         for (int i = 0; i < Q; ++i) acc[i] = 0;
@@ -877,35 +917,38 @@ __device__ __forceinline__ void late_strip(const Smem<Q> &sm, const uint32_t *U,
     }
 }
 
-// helper warp 2: q-row A as soon as the loader has it (rows of the left tile): block K = J-1, into val
+// helper warps: q-row A as soon as the loader has it (rows of the left tile): block K = J-1, into val;
+// warp h takes the columns of q-columns 4h..4h+3
 template <int Q>
-__device__ __forceinline__ void close_row_late(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+__device__ __forceinline__ void close_row_late(const Smem<Q> &sm, const CloseCtx &cc, int h, int lane)
 {
     using C = Cfg<Q>;
-    if (cc.dp == 2)       // K = J-1 = I+1: both operands arrive now; wait for every column of the tile below
-        for (int B = 0; B < 8; ++B) mbar_wait(sm.mbar + C::MB_COL + B, cc.parity);
+    if (cc.dp == 2)       // K = J-1 = I+1: both operands arrive now; wait for my columns of the tile below
+        for (int B = 4 * h; B < 4 * h + 4; ++B) mbar_wait(sm.mbar + C::MB_COL + B, cc.parity);
     for (int A = 7; A >= 0; --A) {
         mbar_wait(sm.mbar + C::MB_ROW + A, cc.parity);
         if (cc.dp >= 2)
-            late_strip<Q>(sm, panel_ZW<Q>(sm), A * Q, cc.dp == 2 ? panel_YX<Q>(sm) : panel_XJ1<Q>(sm), sm.val + 1, C::VP, 1, true, lane);
+            late_strip<Q>(sm, panel_ZW<Q>(sm), A * Q, cc.dp == 2 ? panel_YX<Q>(sm) : panel_XJ1<Q>(sm), 4 * Q * h, 4 * Q * h + 4 * Q,
+                          sm.val + 1, C::VP, 1, true, lane);
         __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + C::MB_RLATE + A);
-        RNA4R_EV(cc, 152 + A);
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_RLATE + 8 * h + A);
+        if (h == 0) RNA4R_EV(cc, 152 + A);
     }
 }
 
-// helper warp 3: q-column B as soon as its closure warp has loaded it (columns of the tile below): block K = I+1, into val2
+// helper warps: q-column B as soon as the loader has it (columns of the tile below): block K = I+1, into val2;
+// warp h takes the rows of q-rows 4h..4h+3 (h = 1, the lower half, is needed first)
 template <int Q>
-__device__ __forceinline__ void close_col_late(const Smem<Q> &sm, const CloseCtx &cc, int lane)
+__device__ __forceinline__ void close_col_late(const Smem<Q> &sm, const CloseCtx &cc, int h, int lane)
 {
     using C = Cfg<Q>;
     for (int B = 0; B < 8; ++B) {
         mbar_wait(sm.mbar + C::MB_COL + B, cc.parity);
         if (cc.dp >= 3)
-            late_strip<Q>(sm, panel_YX<Q>(sm), B * Q, panel_WI1<Q>(sm), sm.val2, 1, C::VP2, false, lane);
+            late_strip<Q>(sm, panel_YX<Q>(sm), B * Q, panel_WI1<Q>(sm), 4 * Q * h, 4 * Q * h + 4 * Q, sm.val2, 1, C::VP2, false, lane);
         __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + C::MB_CLATE + B);
-        RNA4R_EV(cc, 160 + B);
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_CLATE + 8 * h + B);
+        if (h == 1) RNA4R_EV(cc, 160 + B);
     }
 }
 
@@ -1021,9 +1064,12 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         else if (warp < C::NWV + C::NMH) close_mini_helper<Q, false>(sm, cc, warp - C::NWV, lane);
         else if (warp == C::NWV + C::NMH) close_row_loader<Q>(sm, cc, lane);
         else if (warp == C::NWV + C::NMH + 1) close_col_loader<Q>(sm, cc, lane);
-        else if (warp == C::NWV + C::NMH + 2) close_publisher<Q>(sm, cc, lane);
-        else if (warp == C::NWV + C::NMH + 3) close_row_late<Q>(sm, cc, lane);
-        else if (warp == C::NWV + C::NMH + 4) close_col_late<Q>(sm, cc, lane);
+        else if (warp == C::NWV + C::NMH + 2) close_row_late<Q>(sm, cc, 0, lane);
+        else if (warp == C::NWV + C::NMH + 3) close_col_late<Q>(sm, cc, 1, lane);
+        else if (warp == C::NWV + C::NMH + 4) close_publisher<Q>(sm, cc, 1, lane);
+        else if (warp == C::NWV + C::NMH + 5) close_publisher<Q>(sm, cc, 0, lane);
+        else if (warp == C::NWV + C::NMH + 6) close_row_late<Q>(sm, cc, 1, lane);
+        else if (warp == C::NWV + C::NMH + 7) close_col_late<Q>(sm, cc, 0, lane);
         __syncthreads();
         if (tr && tid == 0) tr[4] = global_timer_ns();
     }
@@ -1057,7 +1103,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
 }
 
 template <int Q>
-__global__ void __launch_bounds__(Cfg<Q>::NTHR) fill_kernel(Params p)
+__global__ void __launch_bounds__(Cfg<Q>::NTHR, Cfg<Q>::MIN_CTAS) fill_kernel(Params p)
 {
     using C = Cfg<Q>;
     extern __shared__ __align__(16) uint8_t smem_raw[];
