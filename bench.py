@@ -174,7 +174,13 @@ def main():
     ap.add_argument("--no-also", action="store_true", help="skip the extra workloads (cfg2, cfg4 batch, cfg5)")
     ap.add_argument("--profile", action="store_true", help="short run for ncu: no e2e leg, no tail loop, no extras")
     ap.add_argument("--engine", default="tiled", choices=["tiled", "diag"])
+    ap.add_argument("--cfg", default="cfg3", choices=["cfg2", "cfg3", "cfg5"],
+                    help="single-sequence workload (profiling aid; the headline and the default is cfg3)")
     args = ap.parse_args()
+    global CFG, WORKLOAD
+    if args.cfg != CFG:
+        CFG = args.cfg
+        WORKLOAD = f"{CFG}: single RNA sequence n={workloads.SINGLE_CONFIGS[CFG]['n']}, i.i.d. uniform {{A,C,G,U}}, q=8, score only"
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -331,6 +337,9 @@ def main():
         args.no_also = args.no_cpu = True
     if not args.no_also and world == 1:
         out["also"] = also_workloads(pkg, torch, r, flush)
+        for v in out["also"].values():      # the same shared-memory-gather roofline for the throughput-bound configs
+            if "lookups" in v and v.get("fill_kernel_ms"):
+                v["smem_roofline_frac"] = v["lookups"] / (v["fill_kernel_ms"] * 1e-3) / peak_lookups
     if not args.no_cpu and world == 1:
         base, extra = cpu_baselines(seq, Q)
         out["cpu_baseline"] = base

@@ -8,7 +8,7 @@
 
 namespace {
 
-constexpr int kDelta = 4;   // product stages every kDelta steps
+constexpr int kDelta = 0;   // 0: the tiled engine picks the product-stage span from the problem size
 
 inline bool ctx_ok(const rna4r_ctx *c) { return c && c->magic == RNA4R_MAGIC; }
 

@@ -49,7 +49,8 @@ struct Cfg {
     static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
     static constexpr int NTHR = WTHR + 128;    // + 4 helper warps of the closure: loader, publisher, 2 x late products
     static constexpr int MIN_CTAS = (Q <= 8) ? 3 : 1;   // register budget: 3 CTAs per SM while the table is small
-    static constexpr int RPT = 2 * Q;          // rows per thread in the product phase
+    static constexpr int RPT = Q;              // product phase: a thread owns RPT rows x 2 columns (c and c + T/2): the warp-uniform
+    static constexpr int HT = T / 2;           // row words are loaded once for 2*RPT lookups (a broadcast LDS.128 costs 2 wavefronts)
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
     static constexpr int VP = T + 1;           // pitch of the value array (int16): a wavefront step is conflict-free
     static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
@@ -156,17 +157,20 @@ __host__ __device__ inline int tri_index(int nt, int I, int J) { return I * nt -
 template <int Q>
 __global__ void plan_seq_kernel(Params p)
 {
+    // block <-> sequence; threads <-> steps
     constexpr int T = Cfg<Q>::T;
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int t = blockIdx.x;
     if (t >= p.count) return;
     const int n = p.offsets ? (int)(p.offsets[t + 1] - p.offsets[t]) : p.n_single;
     const int nt = n / T + 1;
-    SeqInfo si;
-    si.n = n; si.nt = nt; si.invalid = 0; si.pad[0] = si.pad[1] = si.pad[2] = 0;
-    si.sbase = atomicAdd(&p.hdr->ntiles, nt * (nt + 1) / 2);
-    si.cbase = atomicAdd(&p.hdr->ncodes, nt * T);
-    p.seqinfo[t] = si;
-    for (int D = 0; D < nt; ++D) {
+    if (threadIdx.x == 0) {
+        SeqInfo si;
+        si.n = n; si.nt = nt; si.invalid = 0; si.pad[0] = si.pad[1] = si.pad[2] = 0;
+        si.sbase = atomicAdd(&p.hdr->ntiles, nt * (nt + 1) / 2);
+        si.cbase = atomicAdd(&p.hdr->ncodes, nt * T);
+        p.seqinfo[t] = si;
+    }
+    for (int D = threadIdx.x; D < nt; D += blockDim.x) {
         atomicAdd(&p.stepC[D], nt - D);
         int np = 0;
         for (int s = 0;; ++s) {
@@ -333,39 +337,41 @@ __device__ __forceinline__ void load_operands_async(const Params &p, const Smem<
     cp_async_commit();
 }
 
-// bulk step (a4): acc[rr] = max over the 8 groups of block K, for column jj and rows rb*RPT+rr.
+// bulk step (a4): acc[h][rr] = max over the 8 groups of block K, for columns cj + h*T/2 and rows rb*RPT+rr.
 // acc is kept in the tagged form (value << SH | low bits); unsigned max orders by value.
 template <int Q>
-__device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, uint32_t (&acc)[Cfg<Q>::RPT], int jj, int rb)
+__device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, uint32_t (&acc)[2][Cfg<Q>::RPT], int cj, int rb)
 {
     using C = Cfg<Q>;
     const uint32_t *PH = sm.stg + (size_t)buf * 2 * C::PANEL_WORDS;
     const uint32_t *PV = PH + C::PANEL_WORDS;
 #pragma unroll 2
     for (int g = 0; g < 8; ++g) {
-        const uint32_t X = PV[g * C::T + jj];
+        const uint32_t X0 = PV[g * C::T + cj], X1 = PV[g * C::T + cj + C::HT];
         const uint32_t *wrow = PH + g * C::T + rb * C::RPT;
         uint32_t w[C::RPT];
-        // the row words are warp-uniform: broadcast vector loads (16 B when RPT % 4 == 0, else 8 B)
+        // the row words are warp-uniform: broadcast vector loads
         if constexpr (C::RPT % 4 == 0) {
 #pragma unroll
             for (int r4 = 0; r4 < C::RPT / 4; ++r4) {
                 const uint4 t4 = reinterpret_cast<const uint4 *>(wrow)[r4];
                 w[4 * r4] = t4.x; w[4 * r4 + 1] = t4.y; w[4 * r4 + 2] = t4.z; w[4 * r4 + 3] = t4.w;
             }
-        } else {
+        } else if constexpr (C::RPT % 2 == 0) {
 #pragma unroll
             for (int r2 = 0; r2 < C::RPT / 2; ++r2) {
                 const uint2 t2 = reinterpret_cast<const uint2 *>(wrow)[r2];
                 w[2 * r2] = t2.x; w[2 * r2 + 1] = t2.y;
             }
+        } else {
+#pragma unroll
+            for (int rr = 0; rr < C::RPT; ++rr) w[rr] = wrow[rr];
         }
 #pragma unroll
         for (int rr = 0; rr < C::RPT; ++rr) {
-            const uint32_t S = w[rr] + X;
-            const uint32_t rv = tbl_gather<Q>(sm, S);
-            const uint32_t cand = S + (rv << C::SH);
-            acc[rr] = max(acc[rr], cand);
+            const uint32_t S0 = w[rr] + X0, S1 = w[rr] + X1;
+            acc[0][rr] = max(acc[0][rr], S0 + (tbl_gather<Q>(sm, S0) << C::SH));
+            acc[1][rr] = max(acc[1][rr], S1 + (tbl_gather<Q>(sm, S1) << C::SH));
         }
     }
 }
@@ -383,10 +389,10 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
     const int lo = max(hi - p.delta + 1, (dp + 1) / 2);
     const int sidx = si.sbase + tri_index(nt, I, J);
     const bool pact = tid < C::PTHR;             // threads beyond 4T only help with barriers (q < 8)
-    const int jj = tid % C::T, rb = pact ? tid / C::T : 0;
-    uint32_t acc[C::RPT];
+    const int cj = tid % C::HT, rb = pact ? tid / C::HT : 0;
+    uint32_t acc[2][C::RPT];
 #pragma unroll
-    for (int rr = 0; rr < C::RPT; ++rr) acc[rr] = 0;
+    for (int rr = 0; rr < C::RPT; ++rr) acc[0][rr] = acc[1][rr] = 0;
 
     // K sequence: for m = lo..hi: K = I+m, then K = J-m (if different)
     const int nk_max = 2 * (hi - lo + 1);
@@ -417,7 +423,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
         const bool more = issue_next();
         if (more) cp_async_wait<1>(); else cp_async_wait<0>();
         __syncthreads();
-        if (pact) product_accumulate<Q>(sm, computed & 1, acc, jj, rb);
+        if (pact) product_accumulate<Q>(sm, computed & 1, acc, cj, rb);
         ++computed;
         __syncthreads();     // the buffer may be refilled by the next issue
     }
@@ -429,15 +435,19 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
         if (pact) {
 #pragma unroll
             for (int rr = 0; rr < C::RPT; ++rr) {
-                const int prev = __ldcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj);
-                acc[rr] = max(acc[rr], (uint32_t)prev << C::SH);
+                const int16_t *row = accg + (size_t)(rb * C::RPT + rr) * C::T + cj;
+                acc[0][rr] = max(acc[0][rr], (uint32_t)(int)__ldcg(row) << C::SH);
+                acc[1][rr] = max(acc[1][rr], (uint32_t)(int)__ldcg(row + C::HT) << C::SH);
             }
         }
     }
     if (pact) {
 #pragma unroll
-        for (int rr = 0; rr < C::RPT; ++rr)
-            __stcg(accg + (size_t)(rb * C::RPT + rr) * C::T + jj, (int16_t)(acc[rr] >> C::SH));
+        for (int rr = 0; rr < C::RPT; ++rr) {
+            int16_t *row = accg + (size_t)(rb * C::RPT + rr) * C::T + cj;
+            __stcg(row, (int16_t)(acc[0][rr] >> C::SH));
+            __stcg(row + C::HT, (int16_t)(acc[1][rr] >> C::SH));
+        }
     }
     __threadfence();
     __syncthreads();
@@ -1138,6 +1148,15 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, Cfg<Q>::MIN_CTAS) fill_kernel(Pa
 // ------------------------------------------------------------------------------------------------
 // host side: workspace layout and enqueue
 // ------------------------------------------------------------------------------------------------
+// Member diagonals per product stage: longer stages mean fewer merge passes over the acc tile (they pay off on
+// long folds, measured at n = 16384), shorter ones feed the closures earlier.
+static inline int pick_delta(int T, const int32_t *lens, int count, int n_single)
+{
+    int max_n = 0;
+    for (int t = 0; t < count; ++t) { const int n = lens ? lens[t] : n_single; if (n > max_n) max_n = n; }
+    return (max_n / T + 1 > 128) ? 8 : 4;
+}
+
 struct HostPlan {
     size_t tiles, codes, tasks;
     int max_nt;
@@ -1191,7 +1210,8 @@ template <int Q>
 static size_t workspace_bytes_q(int delta, const int32_t *lens, int count, int n_single)
 {
     using C = Cfg<Q>;
-    const HostPlan h = host_plan(C::T, delta, lens, count, n_single);
+    (void)delta;
+    const HostPlan h = host_plan(C::T, 4, lens, count, n_single);      // the shortest stage span gives the most tasks: sized for it
     return ws_layout(C::T, C::REC_BYTES, h, count).total;
 }
 
@@ -1200,7 +1220,8 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
                      int count, int n_single, int32_t *scores, void *table_out, int table_dtype, void *ws, cudaStream_t st)
 {
     using C = Cfg<Q>;
-    const HostPlan h = host_plan(C::T, delta, lens_host, count, n_single);
+    if (delta <= 0) delta = pick_delta(C::T, lens_host, count, n_single);
+    const HostPlan h = host_plan(C::T, 4, lens_host, count, n_single);  // layout as sized by workspace_bytes_q
     const WsLayout w = ws_layout(C::T, C::REC_BYTES, h, count);
     char *base = (char *)ws;
     Params p;
@@ -1232,7 +1253,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     }
     int launches = 0;
     RNA4R_CUDA(ctx, cudaMemsetAsync(ws, 0, w.zero_bytes, st));
-    plan_seq_kernel<Q><<<(count + 127) / 128, 128, 0, st>>>(p); ++launches;
+    plan_seq_kernel<Q><<<count, 64, 0, st>>>(p); ++launches;
     plan_scan_kernel<<<1, 32, 0, st>>>(p); ++launches;
     plan_fill_kernel<Q><<<count * h.max_nt, 64, 0, st>>>(p); ++launches;
     {
