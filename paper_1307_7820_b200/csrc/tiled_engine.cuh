@@ -455,20 +455,22 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA): one warp per q-tile column
+// closure of one super-tile (steps a3, a5, a6, a7 inside the CTA)
 //
 // Local coordinates: rows a = 0..T-1 (a = T-1 is the bottom row), columns c = 0..T-1; the super-tile
-// is 8 x 8 q-tiles (A,B) of Q x Q cells.  Warp B owns q-tile column B and walks it bottom-up,
-// A = 7..0; q-tile (A,B) needs (A+1,B) (the warp's own previous one) and (A,B-1) (warp B-1, awaited
-// through a progress counter in shared memory), so the warps form a skewed pipeline: the q-tiles of
-// one anti-diagonal (7-A)+B run together and the super-tile takes 15 q-tile steps
-// (PAPER.md:223-245 wavefront, PAPER.md:291 tiles of one diagonal are independent).
+// is 8 x 8 q-tiles (A,B) of Q x Q cells.  q-tile (A,B) needs (A+1,B) and (A,B-1): the q-tiles of one
+// anti-diagonal u = (7-A)+B are independent and run together as a "macro-step" (15 per super-tile;
+// PAPER.md:223-245 wavefront, PAPER.md:291 tiles of one diagonal are independent).  The CTA's warps take
+// roles: closure warps (G q-tiles side by side per warp, Q lanes each), mini helpers,
+// loaders, late-product helpers, publishers; the closure warps and the mini helpers meet at a named
+// barrier twice per macro-step, everything else is ordered by shared-memory mbarriers.
 //
-// Per q-tile, two phases:
-//  (M) mini-products, all 32 lanes: every group that is complete for the whole q-tile -- z in
-//      [A+1, 7] of block I (column words of the q-tiles below, row words of (I,I)) and z in [8, 8+B-1]
-//      of block J (row words of the q-tiles to the left, column words of (J,J)) -- is one lookup per
-//      cell (full groups), merged into val[][].
+// Per q-tile:
+//  (M) every group that is complete for the whole q-tile -- z in [A+1, 7] of block I (column words of the
+//      q-tiles below, row words of (I,I)) and z in [8, 8+B-1] of block J (row words of the q-tiles to the
+//      left, column words of (J,J)) -- is one lookup per cell (full groups).  The two
+//      groups that were finished in the previous macro-step are looked up in phase F (qtile_fresh_merge),
+//      the older ones one macro-step ahead by the mini helpers (into val3).
 //  (C) cell wavefront, lane y <-> column BQ+y, 2Q skewed steps, lane y one row below lane y-1.  Of all
 //      candidates of cell (a,c) only two depend on the previous step:
 //        left  = v(a,c-1)  (tail split t = c-1: M(r,c-1) + M(c-1,c), M(c-1,c) = 0)   -- one shuffle
@@ -480,7 +482,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 //      ("oldx") and enters v(a-1,c) one step later: the dependent chain of a step is shuffle -> max.
 //      Head and tail are the paper's residual loops done as masked
 //      lookups: not yet known difference bits are zero (DESIGN.md 4.3 proves this is exact).
-// DIAG (I == J): row and column words are both the tile's own (z < 8 only); warp B starts at A = B;
+// DIAG (I == J): row and column words are both the tile's own (z < 8 only); macro-steps start at u = 7;
 // in q-tile (B,B) head and tail are ONE lookup (row word through c-2, Xp); cells with c-a <= 1 are 0.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
