@@ -312,9 +312,20 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// Polls are relaxed loads (an acquire load also invalidates the L1 on every iteration); one acquire load
+// orders the data reads after the flag has been seen.
+__device__ __forceinline__ int ld_relaxed_gpu(const int *p)
+{
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void wait_flag_ge(const int *flag, int v)
 {
-    while (ld_acquire_gpu(flag) < v) __nanosleep(40);
+    if (ld_acquire_gpu(flag) >= v) return;
+    unsigned ns = 64;
+    while (ld_relaxed_gpu(flag) < v) { __nanosleep(ns); if (ns < 512) ns *= 2; }
+    (void)ld_acquire_gpu(flag);
 }
 
 template <int Q>
@@ -651,7 +662,13 @@ struct CloseCtx {
 
 __device__ __forceinline__ void warp_wait_flag_ge(const int *flag, int v, int lane)
 {
-    if (lane == 0) { unsigned ns = 20; while (ld_acquire_gpu(flag) < v) { __nanosleep(ns); if (ns < 160) ns *= 2; } }
+    if (lane == 0) {
+        if (ld_acquire_gpu(flag) < v) {
+            unsigned ns = 32;
+            while (ld_relaxed_gpu(flag) < v) { __nanosleep(ns); if (ns < 256) ns *= 2; }
+            (void)ld_acquire_gpu(flag);
+        }
+    }
     __syncwarp();
 }
 
@@ -751,7 +768,6 @@ __device__ __forceinline__ void close_wave(const Smem<Q> &sm, const CloseCtx &cc
 #pragma unroll 1
     for (int u = DIAG ? 7 : 0; u < 15; ++u) {
         const long long c0 = clock64();
-        if (!DIAG) step_waits<Q>(sm, cc, u);
         macro_fresh<Q, DIAG>(sm, cc, u, w, lane);
         named_bar_sync(1, C::STEP_THREADS);
         const long long c1 = clock64();
@@ -787,10 +803,13 @@ __device__ __forceinline__ void close_mini_helper(const Smem<Q> &sm, const Close
         uint32_t *z = reinterpret_cast<uint32_t *>(sm.val3);
         for (int e = h * 32 + lane; e < C::VAL2_BYTES / 4; e += C::NMH * 32) z[e] = 0;
     }
+    // What a macro-step needs from the loaders and late-product helpers is awaited by mini helper 0 alone, one
+    // macro-step ahead and after its own work (an mbarrier test costs ~90 cycles even when it has completed);
+    // the named barrier that closes the macro-step hands the guarantee to everybody.
+    if (!DIAG && h == 0) step_waits<Q>(sm, cc, 0);
     named_bar_sync(1, C::STEP_THREADS);
 #pragma unroll 1
     for (int u = DIAG ? 7 : 0; u < 15; ++u) {
-        if (!DIAG) step_waits<Q>(sm, cc, u);
         macro_fresh<Q, DIAG>(sm, cc, u, C::NWV + h, lane);
         named_bar_sync(1, C::STEP_THREADS);
         if (u + 1 < 15) {
@@ -800,6 +819,7 @@ __device__ __forceinline__ void close_mini_helper(const Smem<Q> &sm, const Close
                 qtile_of(u + 1, t, A, B);
                 qtile_groups<Q>(sm, A, B, sm.Wst, C::TP, sm.Xst, C::TP, A + 2, ZOFF + B - 2, lane, false, true);
             }
+            if (!DIAG && h == 0) step_waits<Q>(sm, cc, u + 1);
         }
         named_bar_sync(1, C::STEP_THREADS);
     }
@@ -819,7 +839,7 @@ __device__ __forceinline__ void close_col_loader(const Smem<Q> &sm, const CloseC
         // corner M((I+1)T, JT-1) = top row of (I+1,J-1) at its last column
         int corner = 0;
         if (cc.recC) {
-            while (ld_acquire_gpu(cc.doneC) < 1) __nanosleep(40);
+            wait_flag_ge(cc.doneC, 1);
             corner = __ldcg(reinterpret_cast<const uint16_t *>(cc.recC + 2 * C::PANEL_WORDS * 4) + T - 1);
         }
         sm.val[T * VP] = (int16_t)corner;
@@ -985,7 +1005,11 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
     }
     // roles by warp, counted from the top: the SM's issue arbiter favours high warp ids, and the closure
     // warps carry the critical path
-    const int warp = (C::NTHR / 32 - 1) - (tid >> 5), lane = tid & 31;
+    // co-resident CTAs (block index apart by a multiple of the SM count) rotate the roles by two warps, so that
+    // their closure warps land on different SM sub-partitions (warp id mod 4)
+    constexpr int NWARP = C::NTHR / 32;
+    const int rot = 2 * ((blockIdx.x / 148) % 2);
+    const int warp = ((NWARP - 1) - (tid >> 5) + NWARP - rot) % NWARP, lane = tid & 31;
     CloseCtx cc;
     cc.dp = dp;
     cc.parity = (uint32_t)sm.misc[1] & 1u;    // closures this CTA has run so far: phase of its mbarriers
