@@ -11,10 +11,14 @@
 //     max_{t in g} M(r,t)+M(t,c) = M(r,gq) + M(gq,c) + Rc[h][v]
 //   h = the q-1 horizontal difference bits of M(r,gq..gq+q-1)  (v_1..v_{q-1};  v_0 = 0)
 //   v = the q-1 vertical   difference bits of M(gq..gq+q-1,c)  (|vbar_1|..|vbar_{q-1}|; vbar_0 = 0)
-// Each (row, group) is one 32-bit word  W = M(r,gq) << SH | h << HB  and each (group, column) one
-// word X = M(gq,c) << SH | v  (HB = q-1, SH = 2*HB).  Then S = W + X carries the table index in its
-// low SH bits and the anchor sum above them, and  S + (Rc[idx] << SH)  is the candidate, still
-// tagged with harmless low bits: one add, one mask, one byte gather, one shift-add, one max.
+// Each (row, group) is one 32-bit word W = anchor M(r,gq) + index bits h, and each (group, column) one word
+// X = anchor M(gq,c) + index bits v  (HB = q-1 bits each, SH = 2*HB index bits, h above v).  Then S = W + X
+// carries the table index and the anchor sum in disjoint fields, and the candidate is S + Rc[idx] on the value
+// field.  Two layouts (Cfg::F16): q <= 9 keeps the value in the low halfword and the index in the high one, so
+// that the gather address is (S >> 16) + base (one LEA.HI) and "max(acc, S + rv)" is one DPX instruction
+// (VIADDMNMX.U16x2) -- add, address, LDS.U8, add-max; q = 10 (18 index bits) keeps the index in the low SH bits
+// and the value above them (S + (rv << SH), unsigned max).  The index bits left in a candidate are harmless:
+// they never change the order of the value field.
 //
 // Decomposition.  Super-tiles of T = 8q cells (8 groups) per side.  For super-tile (I,J), I < J:
 //   * every group lying in a block K strictly between I and J is a "full group" for ALL T*T cells
@@ -39,12 +43,16 @@ struct Cfg {
     static constexpr int HB = Q - 1;           // informative bits per vector
     static constexpr int SH = 2 * HB;          // table index bits
     static constexpr uint32_t IDXMASK = (1u << SH) - 1u;
+    // Word format.  F16 (q <= 9): value in bits [0,16), table index in bits [16,16+SH): a candidate is
+    // max(acc, S + rv) on the low halfword -- ONE DPX instruction (VIADDMNMX.U16x2; the high halfword carries
+    // harmless index bits), and the gather address is (S >> 16) + base -- one LEA.HI.  q = 10 needs 18 index
+    // bits: index in bits [0,SH), value above (S + (rv << SH), plain unsigned max).
+    static constexpr bool F16 = (SH <= 16);
+    static constexpr int VSHIFT = F16 ? 0 : SH;      // position of the value field
+    static constexpr int ISHIFT = F16 ? 16 : 0;      // position of the index field
     static constexpr bool NIBBLE = (SH > 16);  // q = 10: nibble-packed table (128 KB)
     static constexpr int TBL_BYTES = NIBBLE ? (1 << SH) / 2 : (1 << SH);
-    // q <= 8: the byte table sits at a shared-memory address aligned to its size, so that the gather
-    // address is (S & IDXMASK) | base -- one LOP3 -- instead of mask + add
-    static constexpr bool TBL_ALIGNED = (Q <= 8);
-    static constexpr int TBL_ALIGN = TBL_ALIGNED ? (TBL_BYTES < 16 ? 16 : TBL_BYTES) : 16;
+    static constexpr int TBL_AREA = (TBL_BYTES + 15) / 16 * 16;
     static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
     static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
     static constexpr int NTHR = WTHR + 128;    // + 4 helper warps of the closure: loader, publisher, 2 x late products
@@ -56,7 +64,7 @@ struct Cfg {
     static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
     static constexpr int REC_BYTES = 2 * PANEL_WORDS * 4 + 2 * T * 2;   // PH, PV, top row, right column
     static constexpr int WROWS = 16;           // word-array rows: 8 groups of block I, 8 of block J
-    // shared-memory layout: [guard | Wst | Xst | pad | tbl (aligned) | val (guard rows around) | stg | codeR | codeC | misc | mbar]
+    // shared-memory layout: [tbl | guard | Wst | Xst | val (guard rows around) | val2 | val3 | stg | codeR | codeC | misc | mbar]
     // The unrolled closure steps address val and Wst with immediate offsets; lanes outside their window
     // read up to Q rows beyond either end of the arrays (values ignored): the guards keep those reads inside.
     static constexpr int W_GUARD = 64;         // bytes before Wst
@@ -82,13 +90,11 @@ struct Cfg {
     static constexpr int MBAR_BYTES = MB_COUNT * 8;
     static_assert(NROLE * 32 <= NTHR, "closure roles must fit the CTA");
     static constexpr int POST_BYTES = VAL_BYTES + 2 * VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
-    // dynamic shared memory needed when the dynamic window starts at shared address `base`
-    static constexpr size_t smem_bytes_for(size_t base)
-    {
-        const size_t tbl_at = (base + PRE_BYTES + TBL_ALIGN - 1) / TBL_ALIGN * TBL_ALIGN;
-        return tbl_at - base + (size_t)((TBL_BYTES + 15) / 16 * 16) + POST_BYTES;
-    }
-    static constexpr size_t SMEM_BYTES = smem_bytes_for(0) > smem_bytes_for(1024) ? smem_bytes_for(0) : smem_bytes_for(1024);
+    // The table sits at the START of the dynamic window.  F16: the gather address is (S >> 16) + base with no
+    // mask; an idle lane's don't-care S can index up to 65535, so the window is at least 64 KB + 16 long and the
+    // stray read stays inside it (its value is ignored).
+    static constexpr size_t LAYOUT_BYTES = (size_t)TBL_AREA + PRE_BYTES + POST_BYTES;
+    static constexpr size_t SMEM_BYTES = (F16 && LAYOUT_BYTES < 65536 + 16) ? 65536 + 16 : LAYOUT_BYTES;
 };
 
 struct SeqInfo {
@@ -248,7 +254,7 @@ struct Smem {
     uint32_t *Wst;       // [WROWS][TP] row words:    groups 0..7 of block I (static), 8..15 of block J (own)
     uint32_t *Xst;       // [WROWS][TP] column words: groups 0..7 of block I (own),    8..15 of block J (static)
     uint8_t *tbl;        // compact table Rc
-    uint32_t tbl_sa;     // its shared-space address (aligned to TBL_ALIGN)
+    uint32_t tbl_sa;     // its shared-space address
     int16_t *valraw;     // start of the value array including its guard rows
     int16_t *val;        // [(T+1)][VP] values; column 0 = right column of (I,J-1), row T = top row of (I+1,J)
     int16_t *val2;       // [T][VP2] late products of block K = I+1 (written by the column-late helper, merged by the closure warps)
@@ -262,13 +268,11 @@ struct Smem {
     __device__ explicit Smem(uint8_t *base)
     {
         uint8_t *p = base;
+        tbl = p; tbl_sa = smem_addr(base); p += C::TBL_AREA;
         p += C::W_GUARD;
         Wst = (uint32_t *)p; p += C::W_BYTES;
         Xst = (uint32_t *)p; p += C::W_BYTES;
-        const uint32_t sa0 = smem_addr(base);
-        const uint32_t tsa = (sa0 + C::PRE_BYTES + C::TBL_ALIGN - 1) / C::TBL_ALIGN * C::TBL_ALIGN;
-        p = base + (tsa - sa0);
-        tbl = p; tbl_sa = tsa; p += (C::TBL_BYTES + 15) / 16 * 16;
+        p = base + C::TBL_AREA + C::PRE_BYTES;
         valraw = (int16_t *)p; val = valraw + Q * C::VP; p += C::VAL_BYTES;     // val[0] = row 0; Q guard rows on either side
         val2 = (int16_t *)p; p += C::VAL2_BYTES;
         val3 = (int16_t *)p; p += C::VAL2_BYTES;
@@ -280,12 +284,13 @@ struct Smem {
         mbar = (uint64_t *)p; p += C::MBAR_BYTES;
         uint32_t dyn;
         asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
-        ok = (uint32_t)(p - base) <= dyn;
+        ok = (uint32_t)(p - base) <= dyn && dyn >= (uint32_t)C::SMEM_BYTES;
     }
 };
 
-// One table gather (the unit of work of this path): rv = Rc[S & IDXMASK].
-template <int Q>
+// One table gather (the unit of work of this path): rv = Rc[index field of S].  SAFE marks the call sites where
+// S may be a don't-care value of an idle lane (q = 10 masks the index anyway; F16 relies on the window size).
+template <int Q, bool SAFE = false>
 __device__ __forceinline__ uint32_t tbl_gather(const Smem<Q> &sm, uint32_t S)
 {
     using C = Cfg<Q>;
@@ -293,14 +298,28 @@ __device__ __forceinline__ uint32_t tbl_gather(const Smem<Q> &sm, uint32_t S)
         const uint32_t idx = S & C::IDXMASK;
         const uint32_t w = reinterpret_cast<const uint32_t *>(sm.tbl)[idx >> 3];
         return (w >> ((idx & 7u) * 4u)) & 15u;
-    } else if constexpr (C::TBL_ALIGNED) {
+    } else if constexpr (C::F16) {
+        const uint32_t idx = S >> 16;                 // no mask: see Cfg::SMEM_BYTES
         uint32_t rv;
-        const uint32_t a = (S & C::IDXMASK) | sm.tbl_sa;          // one LOP3: the table is aligned to its size
-        asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"(a));
+        asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"(idx + sm.tbl_sa));
         return rv;
     } else {
         return sm.tbl[S & C::IDXMASK];
     }
+}
+
+// tagged values: (value << VSHIFT) | don't-care bits of the index field
+template <int Q> __device__ __forceinline__ uint32_t tag_value(int v) { return (uint32_t)v << Cfg<Q>::VSHIFT; }
+template <int Q> __device__ __forceinline__ int untag(uint32_t x) { return Cfg<Q>::F16 ? (int)(x & 0xffffu) : (int)(x >> Cfg<Q>::SH); }
+template <int Q> __device__ __forceinline__ uint32_t tag_max(uint32_t a, uint32_t b) { return Cfg<Q>::F16 ? __vmaxu2(a, b) : max(a, b); }
+
+// acc = max(acc, candidate of the word sum S): eq. (3)
+template <int Q, bool SAFE = false>
+__device__ __forceinline__ uint32_t lookup_max(const Smem<Q> &sm, uint32_t S, uint32_t acc)
+{
+    const uint32_t rv = tbl_gather<Q, SAFE>(sm, S);
+    if constexpr (Cfg<Q>::F16) return __viaddmax_u16x2(S, rv, acc);
+    else return max(acc, S + (rv << Cfg<Q>::SH));
 }
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
@@ -349,7 +368,7 @@ __device__ __forceinline__ void load_operands_async(const Params &p, const Smem<
 }
 
 // bulk step (a4): acc[h][rr] = max over the 8 groups of block K, for columns cj + h*T/2 and rows rb*RPT+rr.
-// acc is kept in the tagged form (value << SH | low bits); unsigned max orders by value.
+// acc is kept in the tagged form (value field + don't-care index bits); tag_max orders by value.
 template <int Q>
 __device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, uint32_t (&acc)[2][Cfg<Q>::RPT], int cj, int rb)
 {
@@ -381,8 +400,8 @@ __device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, u
 #pragma unroll
         for (int rr = 0; rr < C::RPT; ++rr) {
             const uint32_t S0 = w[rr] + X0, S1 = w[rr] + X1;
-            acc[0][rr] = max(acc[0][rr], S0 + (tbl_gather<Q>(sm, S0) << C::SH));
-            acc[1][rr] = max(acc[1][rr], S1 + (tbl_gather<Q>(sm, S1) << C::SH));
+            acc[0][rr] = lookup_max<Q>(sm, S0, acc[0][rr]);
+            acc[1][rr] = lookup_max<Q>(sm, S1, acc[1][rr]);
         }
     }
 }
@@ -447,8 +466,8 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 #pragma unroll
             for (int rr = 0; rr < C::RPT; ++rr) {
                 const int16_t *row = accg + (size_t)(rb * C::RPT + rr) * C::T + cj;
-                acc[0][rr] = max(acc[0][rr], (uint32_t)(int)__ldcg(row) << C::SH);
-                acc[1][rr] = max(acc[1][rr], (uint32_t)(int)__ldcg(row + C::HT) << C::SH);
+                acc[0][rr] = tag_max<Q>(acc[0][rr], tag_value<Q>((int)__ldcg(row)));
+                acc[1][rr] = tag_max<Q>(acc[1][rr], tag_value<Q>((int)__ldcg(row + C::HT)));
             }
         }
     }
@@ -456,8 +475,8 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 #pragma unroll
         for (int rr = 0; rr < C::RPT; ++rr) {
             int16_t *row = accg + (size_t)(rb * C::RPT + rr) * C::T + cj;
-            __stcg(row, (int16_t)(acc[0][rr] >> C::SH));
-            __stcg(row + C::HT, (int16_t)(acc[1][rr] >> C::SH));
+            __stcg(row, (int16_t)untag<Q>(acc[0][rr]));
+            __stcg(row + C::HT, (int16_t)untag<Q>(acc[1][rr]));
         }
     }
     __threadfence();
@@ -517,12 +536,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
 }
 
-template <int Q>
-__device__ __forceinline__ uint32_t lookup_tagged(const Smem<Q> &sm, uint32_t S)
-{
-    return S + (tbl_gather<Q>(sm, S) << Cfg<Q>::SH);      // (value << SH) | harmless low bits
-}
-
 // Complete-group lookups for the Q x Q cells of q-tile (A,B), all 32 lanes: for z in [zlo, zhi],
 // val[a][c] = max(val[a][c], lookup(W[z*wp + a] + X[z*xp + c])).  Used for the mini-products of the
 // closure (W = Wst, X = Xst) and for the late products (operand panels of the neighbouring blocks).
@@ -548,17 +561,17 @@ __device__ __forceinline__ void qtile_groups(const Smem<Q> &sm, int A, int B, co
         for (int i = 0; i < NX; ++i) {
             const int x = xr + i * RS;
             const int a = abot - (x < Q ? x : 0);
-            best[i] = max(best[i], lookup_tagged<Q>(sm, W[z * wp + a] + Xw));
+            best[i] = lookup_max<Q>(sm, W[z * wp + a] + Xw, best[i]);
         }
     }
 #pragma unroll
     for (int i = 0; i < NX; ++i) {
         const int x = xr + i * RS;
         if (x < Q && out3) {
-            sm.val3[(abot - x) * C::VP2 + mc] = (int16_t)(best[i] >> SH);        // written once per cell
+            sm.val3[(abot - x) * C::VP2 + mc] = (int16_t)untag<Q>(best[i]);      // written once per cell
         } else if (x < Q) {
             int16_t *cell = sm.val + (abot - x) * VP + mc + 1;
-            int v = max((int)*cell, (int)(best[i] >> SH));
+            int v = max((int)*cell, untag<Q>(best[i]));
             if (merge2) v = max(v, (int)sm.val2[(abot - x) * C::VP2 + mc]);      // late products of block I+1
             *cell = (int16_t)v;
         }
@@ -580,8 +593,8 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
     const uint32_t w2mask = (y >= 2) ? FULL : 0u;
     const int c = B * Q + y;
     const int abot = A * Q + Q - 1;
-    const int shb = HB + (y > 0 ? y - 1 : 0);            // position of my horizontal difference bit
-    const int sh0 = Q - 1 + y;                           // vertical bit of row x = s-y sits at sh0 - s
+    const int shb = C::ISHIFT + HB + (y > 0 ? y - 1 : 0);   // position of my horizontal difference bit
+    const int sh0 = C::ISHIFT + Q - 2 + y;                  // vertical bit of row x = s-y sits at sh0 - (s-1) (sh0 <= 31)
     const uint32_t XJ = MERGED ? 0u : sm.Xst[(ZOFF + B) * TP + c];
     uint32_t pms = 0;                                    // bit (x + y) <-> row x pairs with my column
     {
@@ -610,7 +623,7 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         const bool live = own && (unsigned)(s - y) < (unsigned)Q;
         if (live) vb[-s * VP] = (int16_t)v;
         // ---- step a6, horizontal: my row word = neighbour's word | my difference bit
-        const uint32_t vnew = (uint32_t)v << SH;
+        const uint32_t vnew = tag_value<Q>(v);
         const uint32_t wme = firstcol ? vnew : (Lw | ((uint32_t)(v - Lv) << shb));
         if (live && lastcol) {
             wo[-s] = wme;
@@ -623,15 +636,15 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         uint32_t Xp = xbits + vsh;                                  // running column word: rows >= a+1
         if (s + 1 < Q && y > s) Xp = 0;                             // not in the q-tile yet: no row of it lies below
         if (MERGED) {
-            best = lookup_tagged<Q>(sm, Lw2 + Xp);
+            best = lookup_max<Q, true>(sm, Lw2 + Xp, 0u);
         } else {
-            best = max(lookup_tagged<Q>(sm, wb[-s] + Xp), lookup_tagged<Q>(sm, Lw2 + XJ));
+            best = lookup_max<Q, true>(sm, Lw2 + XJ, lookup_max<Q, true>(sm, wb[-s] + Xp, 0u));
         }
-        oldx = max(o, (int)(best >> SH));
+        oldx = max(o, untag<Q>(best));
         // ---- step a6, vertical: the column word now starts at row a (anchor v, bit of the pair (a, a+1))
         {
-            const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 0 ? s : 0) & 31);
-            xbits = (y <= s - 1) ? ((xbits | dbit) & C::IDXMASK) : 0u;     // x >= 1
+            const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 1 ? s - 1 : 0) & 31);   // used for x >= 1 only
+            xbits = (y <= s - 1) ? ((xbits | dbit) & (C::IDXMASK << C::ISHIFT)) : 0u;     // x >= 1
             vsh = vnew;
         }
         if (x_lo >= 0 && live && y == x_lo) sm.Xst[A * TP + c] = xbits + vsh;    // x = Q-1: the column word is complete
@@ -717,9 +730,9 @@ __device__ __forceinline__ void qtile_fresh_merge(const Smem<Q> &sm, int A, int 
             const int a = abot - x;
             int v = max((int)sm.val[a * VP + c + 1], (int)sm.val3[a * VP2 + c]);
             if (use2) v = max(v, (int)sm.val2[a * VP2 + c]);
-            const uint32_t b1 = lookup_tagged<Q>(sm, (w1[a] & m1) + X1);     // a zero pair looks up R[0][0] = 0
-            const uint32_t b2 = lookup_tagged<Q>(sm, (w2[a] & m2) + X2);
-            v = max(v, (int)(max(b1, b2) >> SH));
+            const uint32_t b1 = lookup_max<Q>(sm, (w1[a] & m1) + X1, 0u);     // a zero pair looks up R[0][0] = 0
+            const uint32_t b2 = lookup_max<Q>(sm, (w2[a] & m2) + X2, b1);
+            v = max(v, untag<Q>(b2));
             sm.val[a * VP + c + 1] = (int16_t)v;
         }
     }
@@ -938,12 +951,12 @@ __device__ __forceinline__ void late_strip(const Smem<Q> &sm, const uint32_t *U,
             const uint32_t Lw = L[g * T + l];
             const uint32_t *u = U + g * T + u0;
 #pragma unroll
-            for (int i = 0; i < Q; ++i) acc[i] = max(acc[i], lookup_tagged<Q>(sm, u[i] + Lw));
+            for (int i = 0; i < Q; ++i) acc[i] = lookup_max<Q>(sm, u[i] + Lw, acc[i]);
         }
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             int16_t *cell = out + (u0 + i) * out_us + l * out_ls;
-            const int v = (int)(acc[i] >> SH);
+            const int v = untag<Q>(acc[i]);
             *cell = (int16_t)(domax ? max((int)*cell, v) : v);
         }
     }
