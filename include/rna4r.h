@@ -175,8 +175,9 @@ int rna4r_last_fill_kernel_ms(rna4r_ctx *ctx, float *ms_host);
  * Wavefront trace (TILED engine; a profiling aid for the per-diagonal latency of step a7).  With
  * max_tiles > 0 the context allocates max_tiles * 64 bytes; every closure task of a later fold then
  * writes eight uint64 for its super-tile (index = order of the triangular enumeration, row-major
- * I <= J): %globaltimer ns at [0] task claimed, [1] dependencies met, [2] operands loaded, [3] late
- * products done, [4] in-tile wavefront done, [5] published; [6] = I << 32 | J; [7] unused.
+ * I <= J): %globaltimer ns at [0] task claimed, [1] static dependencies met, [2],[3] prologue loaded,
+ * [4] closure warp 0 reached the final barrier, [5] record complete and flagged; [6] = I << 32 | J;
+ * [7] = clock64 cycles of closure warp 0 in three 21-bit fields (fresh merge | cell wavefronts | barrier).
  * max_tiles = 0 frees the buffer and switches tracing off.  rna4r_trace_to_host synchronises the
  * device and copies `tiles` records to HOST memory.  Errors: CONTEXT, NULL, BAD_N, CUDA.
  */
