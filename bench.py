@@ -373,6 +373,20 @@ def also_workloads(pkg, torch, r8, flush):
     d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()
     ms = time_call(lambda: r8.fold(d), 10)
     res["cfg2_n2000_q8"] = {"ms": ms, "cell_k_updates_per_s": nussinov_updates(len(s)) / (ms * 1e-3)}
+    # cfg3 with the full int16 table written (72 MB, step a8) and one traceback over it
+    s3 = workloads.single_config("cfg3")
+    d3 = torch.from_numpy(np.frombuffer(s3, dtype=np.uint8).copy()).cuda()
+    tab3 = torch.empty((len(s3), len(s3)), dtype=torch.int16, device="cuda")
+    ms_tab = time_call(lambda: r8.fold(d3, table_dtype=pkg.TABLE_INT16, table_out=tab3), 5)
+    out_tb = {}
+
+    def tb():
+        out_tb["r"] = r8.traceback(d3, tab3)
+
+    ms_tb = time_call(tb, 5)
+    res["cfg3_n6000_q8_with_table"] = {"ms": ms_tab, "table_bytes": int(tab3.numel()) * 2,
+                                        "traceback_ms": ms_tb, "traceback_pairs": int(out_tb["r"][1].item())}
+    del tab3
     # cfg4 batch
     seqs, lens = workloads.gc_rich_batch()
     flat, offsets, lens32 = workloads.pack_batch(seqs)

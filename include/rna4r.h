@@ -143,6 +143,25 @@ int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *off
                      void *workspace_dev, size_t workspace_bytes, void *stream);
 
 /*
+ * rna4r_traceback -- one optimal structure (a maximum set of non-crossing complementary pairs) from a
+ * finished table.  The paper stores arg-max indices beside the maxima (D*); this call
+ * recovers the pairs from D alone by re-running eq. (1) along the optimal path: an interval
+ * pairs its ends if b(S_i,S_j) = 1 and D(i,j) = 1 + D(i+1,j-1), else it splits at the smallest k in [i+1,j]
+ * with D(i,j) = D(i,k-1) + D(k,j).  Deterministic; several structures may be optimal, this rule picks one.
+ *   seq_dev        device uint8[n]: the bases (as given to rna4r_fold).
+ *   table_dev      device n*n elements in the layout rna4r_fold writes (table_dtype INT16 or INT32).
+ *   pairs_out_dev  device int32[n]: partner (0-based) of every base, -1 if unpaired.
+ *   npairs_out_dev device int32[1]: number of pairs = D(1,n); -1 if the sequence holds an invalid byte or the
+ *                  table is not a table of eq. (1) for this sequence.
+ *   workspace_dev  device scratch of >= rna4r_traceback_workspace_bytes(ctx, n) bytes.
+ * Enqueues only (no allocation, no synchronisation).  Errors: CONTEXT, NULL, BAD_N, DTYPE, WORKSPACE, CUDA.
+ */
+size_t rna4r_traceback_workspace_bytes(const rna4r_ctx *ctx, int n);
+int rna4r_traceback(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, const void *table_dev, int table_dtype,
+                    int32_t *pairs_out_dev, int32_t *npairs_out_dev,
+                    void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/*
  * Host-buffer variants (the end-to-end path): the sequence(s) are copied host->device into the
  * workspace, folded, the score(s) (and table) copied device->host, and `stream` is synchronised
  * before returning.  Host buffers should be pinned for full copy bandwidth but need not be.

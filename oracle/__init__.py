@@ -9,6 +9,8 @@ Functions and the passages they follow:
   brute_force_matchings / brute_force_structural -- the definition, PAPER.md:45     (the pins)
   blackbox / rtable                             -- listing PAPER.md:91-113          (pinned)
   two_vector_serial                             -- Algorithm 1, PAPER.md:125-187    (baseline, pinned to eq. (1))
+  structure.check_structure / structure.traceback -- feasibility by the definition; plain
+                                                   traceback of eq. (1), PAPER.md:54, :87 (pinned)
 """
 from __future__ import annotations
 

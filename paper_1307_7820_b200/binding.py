@@ -61,6 +61,9 @@ def load():
     L.rna4r_fold_batch_host.argtypes = [vp, u8p, i32p, ctypes.c_int, i32p, vp, ctypes.c_size_t, vp]
     L.rna4r_enable_kernel_timing.argtypes = [vp, ctypes.c_int]
     L.rna4r_last_fill_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.rna4r_traceback_workspace_bytes.argtypes = [vp, ctypes.c_int]
+    L.rna4r_traceback_workspace_bytes.restype = ctypes.c_size_t
+    L.rna4r_traceback.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp, vp, ctypes.c_size_t, vp]
     L.rna4r_set_trace.argtypes = [vp, ctypes.c_int]
     L.rna4r_trace_to_host.argtypes = [vp, vp, ctypes.c_int]
     L.rna4r_last_launch_count.argtypes = [vp]
@@ -202,6 +205,23 @@ class Rna4r:
                                          scores_out.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                          _stream_ptr(stream)), "rna4r_fold_batch")
         return scores_out[:count]
+
+    # -- traceback --------------------------------------------------------------------------------
+    def traceback(self, seq_dev, table, n: int | None = None, stream=None):
+        """rna4r_traceback.  seq_dev: torch uint8 CUDA tensor; table: the (n, n) int16/int32 CUDA tensor
+        rna4r_fold wrote.  Enqueues only; returns (pairs int32[n] with -1 = unpaired, npairs int32[1])."""
+        import torch
+        n = int(seq_dev.numel()) if n is None else n
+        dev = f"cuda:{self.device}"
+        dt = TABLE_INT16 if table.dtype == torch.int16 else TABLE_INT32
+        pairs = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+        npairs = torch.empty(1, dtype=torch.int32, device=dev)
+        ws = torch.empty(self.lib.rna4r_traceback_workspace_bytes(self.h, n), dtype=torch.uint8, device=dev)
+        _check(self.lib.rna4r_traceback(self.h, seq_dev.data_ptr() if n else None, n, table.data_ptr() if n else None, dt,
+                                        pairs.data_ptr(), npairs.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
+               "rna4r_traceback")
+        self._tb_ws = ws          # keep the scratch alive until the stream has run
+        return pairs[:n], npairs
 
     # -- folds (host buffers; copies inside, synchronises) ---------------------------------------
     def fold_host(self, seq_host, table_dtype: int = TABLE_NONE, workspace=None, stream=None, score_host=None, table_host=None):

@@ -3,6 +3,7 @@
 #include "rtable.cuh"
 #include "diag_engine.cuh"
 #include "tiled_engine.cuh"
+#include "traceback.cuh"
 
 #include <new>
 
@@ -296,6 +297,41 @@ int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *off
         return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
                                                     nullptr, RNA4R_TABLE_NONE, workspace_dev, st);
     });
+}
+
+// ---- traceback: one optimal structure from a finished table ------------------------
+size_t rna4r_traceback_workspace_bytes(const rna4r_ctx *ctx, int n)
+{
+    if (!ctx_ok(ctx) || n < 0 || n > 65534) return 0;
+    return traceback::workspace_bytes(n);
+}
+
+int rna4r_traceback(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, const void *table_dev, int table_dtype,
+                    int32_t *pairs_out_dev, int32_t *npairs_out_dev, void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (n < 0 || n > 65534) return RNA4R_ERR_BAD_N;
+    if (!npairs_out_dev || !workspace_dev || (n > 0 && (!seq_dev || !table_dev || !pairs_out_dev))) return RNA4R_ERR_NULL;
+    if (table_dtype != RNA4R_TABLE_INT16 && table_dtype != RNA4R_TABLE_INT32) return RNA4R_ERR_DTYPE;
+    if (workspace_bytes < traceback::workspace_bytes(n)) return RNA4R_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    traceback::Queue *q = (traceback::Queue *)workspace_dev;
+    unsigned long long *slots = (unsigned long long *)((char *)workspace_dev + 256);
+    const int nslots = 2 * n + 64;
+    traceback::init_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(q, slots, nslots, pairs_out_dev, n);
+    if (n >= 2) {
+        int blocks = ctx->sm_count;
+        if (blocks > (n + 63) / 64) blocks = (n + 63) / 64;       // small folds have few branches
+        if (table_dtype == RNA4R_TABLE_INT16)
+            traceback::walk_kernel<int16_t><<<blocks, 256, 0, st>>>(seq_dev, n, (const int16_t *)table_dev, q, slots, pairs_out_dev);
+        else
+            traceback::walk_kernel<int32_t><<<blocks, 256, 0, st>>>(seq_dev, n, (const int32_t *)table_dev, q, slots, pairs_out_dev);
+    }
+    traceback::finish_kernel<<<1, 32, 0, st>>>(q, npairs_out_dev);
+    RNA4R_CUDA(ctx, cudaGetLastError());
+    ctx->last_launches = n >= 2 ? 3 : 2;
+    return RNA4R_OK;
 }
 
 // ---- host-buffer variants: staging area at the END of the workspace --------------------------------
