@@ -387,6 +387,14 @@ def also_workloads(pkg, torch, r8, flush):
     res["cfg3_n6000_q8_with_table"] = {"ms": ms_tab, "table_bytes": int(tab3.numel()) * 2,
                                         "traceback_ms": ms_tb, "traceback_pairs": int(out_tb["r"][1].item())}
     del tab3
+    # q sweep at n = 6000 (the paper saw the serial gains saturate at q = 8-9)
+    sweep = {}
+    for q in (4, 5, 6, 7, 8, 9, 10):
+        rq = r8 if q == 8 else pkg.Rna4r(q, 0)
+        sweep[str(q)] = time_call(lambda: rq.fold(d3), 5)
+        if q != 8:
+            rq.close()
+    res["q_sweep_n6000_ms"] = sweep
     # cfg4 batch
     seqs, lens = workloads.gc_rich_batch()
     flat, offsets, lens32 = workloads.pack_batch(seqs)
