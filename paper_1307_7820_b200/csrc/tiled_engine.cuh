@@ -37,6 +37,8 @@
 
 namespace tiled {
 
+
+
 template <int Q>
 struct Cfg {
     static constexpr int T = 8 * Q;            // cells per super-tile side
@@ -606,22 +608,48 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
     int16_t *vb = sm.val + (abot + y) * VP + c + 1;                 // vb[-s*VP]  = val[a][c],  a = abot + y - s
     const uint32_t *wb = sm.Wst + A * TP + abot + y - 1;            // wb[-s]     = Wst[A][a-1]
     uint32_t *wo = sm.Wst + (ZOFF + B) * TP + abot + y;             // wo[-s]     = own row word of row a
-    int vprev = 0, oldx = 0;
+    int vprev = 0;
     uint32_t wout = 0, xbits = 0, vsh = 0;
+    // Operands that do not depend on this wavefront (the head row word, the prepared value of the next cell, the
+    // left neighbour's column for lane 0, the cell below the q-tile) are loaded one step ahead: a single warp
+    // issues in order, so a load placed next to its use would add its 29 cycles to every step.
+    const int vbelow = sm.val[(abot + 1) * VP + c + 1];
+    uint32_t w_nxt = wb[1];
+    int o_nxt = vb[0], lv_nxt = vb[VP - 1];
+    // The two lookups of a step are only consumed one step later (they belong to the NEXT cell), so they are
+    // carried as pending (word sum, table byte) pairs and folded in after the next step's shuffles have been
+    // issued: gather latency and shuffle latency overlap instead of adding up.
+    uint32_t hS = 0, hR = 0, tS = 0, tR = 0;
+    int o_pend = 0;
 #pragma unroll
     for (int s = -1; s <= 2 * Q - 2; ++s) {
         const int x_lo = s - (Q - 1);                               // rows touched this step: x in [x_lo, s]
+        const uint32_t w_cur = w_nxt;
+        const int o_cur = o_nxt, lv_cur = lv_nxt;
+        if (s < 2 * Q - 2) { w_nxt = wb[-(s + 1)]; o_nxt = vb[-(s + 2) * VP]; lv_nxt = vb[-(s + 1) * VP - 1]; }
+        // ---- oldx of my cell: fold in the lookups issued in the previous step
+        uint32_t best = 0;
+        if (!MERGED) best = Cfg<Q>::F16 ? __viaddmax_u16x2(hS, hR, 0u) : hS + (hR << SH);
+        best = Cfg<Q>::F16 ? __viaddmax_u16x2(tS, tR, best) : max(best, tS + (tR << SH));
+        // ---- head lookup of the NEXT cell: running column word (rows >= a+1) x row word of group A of block I
+        uint32_t Xp = xbits + vsh;
+        if (s + 1 < Q && y > s) Xp = 0;                             // not in the q-tile yet: no row of it lies below
+        if (!MERGED) { hS = w_cur + Xp; hR = tbl_gather<Q, true>(sm, hS); }
         // ---- receive from the left
         int Lv = __shfl_sync(FULL, vprev, src1);                    // v(a, c-1)
         const uint32_t Lw = __shfl_sync(FULL, wout, src1);          // row a   through column c-1
         const uint32_t Lw2 = __shfl_sync(FULL, wout, src2) & w2mask;   // row a-1 through column c-2
-        if (firstcol) Lv = vb[-s * VP - 1];                         // column c-1 belongs to the q-tile on the left
+        if (firstcol) Lv = lv_cur;                                  // column c-1 belongs to the q-tile on the left
         // ---- the cell (a3 init + a5 fresh splits)
+        const int oldx = max(o_pend, untag<Q>(best));
         int v = max(max(oldx, vprev), Lv);
-        if (s + 1 < Q && y == s + 1) v = vb[-s * VP];               // pre-step (x = -1): the cell below the q-tile
+        if (s + 1 < Q && y == s + 1) v = vbelow;                    // pre-step (x = -1): the cell below the q-tile
         if (MERGED && s - (Q - 1) <= 1) v = 0;                      // D(i,i) = D(i,i-1) = 0
         const bool live = own && (unsigned)(s - y) < (unsigned)Q;
         if (live) vb[-s * VP] = (int16_t)v;
+        // ---- tail lookup of the NEXT cell: row word of row a-1 through column c-2 x column word of group B of block J
+        tS = Lw2 + (MERGED ? Xp : XJ);
+        tR = tbl_gather<Q, true>(sm, tS);
         // ---- step a6, horizontal: my row word = neighbour's word | my difference bit
         const uint32_t vnew = tag_value<Q>(v);
         const uint32_t wme = firstcol ? vnew : (Lw | ((uint32_t)(v - Lv) << shb));
@@ -629,18 +657,8 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
             wo[-s] = wme;
             if (DIAG) wo[-s + 8 * TP] = wme;
         }
-        // ---- oldx of the next cell (a-1, c)
-        int o = vb[-(s + 1) * VP];                                  // bulk + mini-products
-        o = max(o, Lv + (int)((pms >> ((s + 1) & 31)) & 1u));       // b(S_i,S_j) + D(i+1,j-1)
-        uint32_t best;
-        uint32_t Xp = xbits + vsh;                                  // running column word: rows >= a+1
-        if (s + 1 < Q && y > s) Xp = 0;                             // not in the q-tile yet: no row of it lies below
-        if (MERGED) {
-            best = lookup_max<Q, true>(sm, Lw2 + Xp, 0u);
-        } else {
-            best = lookup_max<Q, true>(sm, Lw2 + XJ, lookup_max<Q, true>(sm, wb[-s] + Xp, 0u));
-        }
-        oldx = max(o, untag<Q>(best));
+        // ---- the rest of the next cell's candidates: prepared value, b(S_i,S_j) + D(i+1,j-1)
+        o_pend = max(o_cur, Lv + (int)((pms >> ((s + 1) & 31)) & 1u));
         // ---- step a6, vertical: the column word now starts at row a (anchor v, bit of the pair (a, a+1))
         {
             const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 1 ? s - 1 : 0) & 31);   // used for x >= 1 only
