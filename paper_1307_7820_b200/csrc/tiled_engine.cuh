@@ -85,10 +85,11 @@ struct Cfg {
     static constexpr int NROLE = NWV + NMH + 8;          // + row/column loader, row/column publisher, 2 row-late, 2 column-late
     static constexpr int STEP_THREADS = (NWV + NMH) * 32;   // participants of the per-macro-step named barrier
     // mbarriers (each completes once per closure): [0,15) macro-step u done; [16,24) rows of q-row A of the left
-    // tile loaded; [24,32) columns of q-column B of the tile below loaded; [32,48) late products of q-row A merged
-    // for the left / right half of the columns (32+A, 40+A); [48,64) late products of q-column B merged for the
-    // upper / lower half of the rows (48+B, 56+B)
-    static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_RLATE = 32, MB_CLATE = 48, MB_COUNT = 64;
+    // tile loaded; [24,32) columns of q-column B of the tile below loaded; [32,47) everything macro-step u needs
+    // from the late-product helpers has been merged: the left (right) half of q-row A's late products arrives at
+    // u = 7-A (11-A), the lower (upper) half of q-column B's at u = B (B+4) -- see stepin_count()
+    static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_STEPIN = 32, MB_COUNT = 48;
+    __host__ __device__ static constexpr int stepin_count(int u) { return (u <= 3) ? 2 : (u <= 7) ? 4 : (u <= 11) ? 2 : 0; }
     static constexpr int MBAR_BYTES = MB_COUNT * 8;
     static_assert(NROLE * 32 <= NTHR, "closure roles must fit the CTA");
     static constexpr int POST_BYTES = VAL_BYTES + 2 * VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
@@ -763,14 +764,7 @@ template <int Q>
 __device__ __forceinline__ void step_waits(const Smem<Q> &sm, const CloseCtx &cc, int u)
 {
     using C = Cfg<Q>;
-    if (u <= 7) {
-        mbar_wait(sm.mbar + C::MB_RLATE + 7 - u, cc.parity);
-        mbar_wait(sm.mbar + C::MB_CLATE + 8 + u, cc.parity);
-    }
-    if (u >= 4 && u <= 11) {
-        mbar_wait(sm.mbar + C::MB_RLATE + 8 + 11 - u, cc.parity);
-        mbar_wait(sm.mbar + C::MB_CLATE + u - 4, cc.parity);
-    }
+    if (u <= 11) mbar_wait(sm.mbar + C::MB_STEPIN + u, cc.parity);
 }
 
 // phase F of macro-step u, step warp sw of NWV+NMH
@@ -994,7 +988,7 @@ __device__ __forceinline__ void close_row_late(const Smem<Q> &sm, const CloseCtx
             late_strip<Q>(sm, panel_ZW<Q>(sm), A * Q, cc.dp == 2 ? panel_YX<Q>(sm) : panel_XJ1<Q>(sm), 4 * Q * h, 4 * Q * h + 4 * Q,
                           sm.val + 1, C::VP, 1, true, lane);
         __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + C::MB_RLATE + 8 * h + A);
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_STEPIN + (h == 0 ? 7 - A : 11 - A));
         if (h == 0) RNA4R_EV(cc, 152 + A);
     }
 }
@@ -1010,7 +1004,7 @@ __device__ __forceinline__ void close_col_late(const Smem<Q> &sm, const CloseCtx
         if (cc.dp >= 3)
             late_strip<Q>(sm, panel_YX<Q>(sm), B * Q, panel_WI1<Q>(sm), 4 * Q * h, 4 * Q * h + 4 * Q, sm.val2, 1, C::VP2, false, lane);
         __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + C::MB_CLATE + 8 * h + B);
+        if (lane == 0) mbar_arrive(sm.mbar + C::MB_STEPIN + (h == 1 ? B : B + 4));
         if (h == 1) RNA4R_EV(cc, 160 + B);
     }
 }
@@ -1059,7 +1053,8 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         else if (warp < C::NWV + C::NMH) close_mini_helper<Q, true>(sm, cc, warp - C::NWV, lane);
         else if (warp == C::NWV + C::NMH) {
             // keep the phases of the barriers a diagonal super-tile does not use in step
-            for (int e = lane; e < C::MB_COUNT - C::MB_ROW; e += 32) mbar_arrive(sm.mbar + C::MB_ROW + e);
+            if (lane < 16) mbar_arrive(sm.mbar + C::MB_ROW + lane);
+            if (lane < 12) for (int k = 0; k < C::stepin_count(lane); ++k) mbar_arrive(sm.mbar + C::MB_STEPIN + lane);
             if (lane < 7) mbar_arrive(sm.mbar + C::MB_STEP + lane);
         }
         __syncthreads();
@@ -1184,7 +1179,10 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, Cfg<Q>::MIN_CTAS) fill_kernel(Pa
         for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
         if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
     }
-    if (tid < C::MB_COUNT) mbar_init(sm.mbar + tid, 1);
+    if (tid < C::MB_COUNT) {
+        const int u = tid - C::MB_STEPIN;
+        mbar_init(sm.mbar + tid, (u >= 0 && u < 12) ? C::stepin_count(u) : 1);
+    }
     if (tid == 0) sm.misc[1] = 0;
     __syncthreads();
     const int total = p.hdr->total;
