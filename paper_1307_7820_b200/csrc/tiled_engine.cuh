@@ -532,11 +532,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "{\n"
         ".reg .pred P1;\n"
         "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.acquire.cta.shared.b64 P1, [%0], %1;\n"
+        "mbarrier.try_wait.parity.acquire.cta.shared.b64 P1, [%0], %1, %2;\n"
         "@P1 bra.uni WAIT_DONE;\n"
         "bra.uni WAIT_LOOP;\n"
         "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+        "}\n" ::"r"(smem_addr(bar)), "r"(parity), "r"(20000u) : "memory");     // suspend-time hint (ns): park, do not spin
 }
 
 // Complete-group lookups for the Q x Q cells of q-tile (A,B), all 32 lanes: for z in [zlo, zhi],
