@@ -53,7 +53,15 @@ struct Cfg {
     static constexpr int VSHIFT = F16 ? 0 : SH;      // position of the value field
     static constexpr int ISHIFT = F16 ? 16 : 0;      // position of the index field
     static constexpr bool NIBBLE = (SH > 16);  // q = 10: nibble-packed table (128 KB)
-    static constexpr int TBL_BYTES = NIBBLE ? (1 << SH) / 2 : (1 << SH);
+    // F16: the table rows (2^HB bytes, one per h) are stored with a pitch of 2^HB + 4 bytes.  A row of 128 bytes
+    // covers the 32 banks exactly once, so with the natural pitch the bank of a gather depends on v alone and the
+    // closure's gathers -- different h per lane, partial (mostly zero) v -- pile up on a few banks (ncu: 7-way
+    // conflicts).  With the padded pitch the bank is (h + v/4) mod 32; the bulk product (one h per warp) stays
+    // conflict-free.  The index field of a row word is then h * TBL_PITCH (a sum of per-bit constants), not a
+    // bit field; the column word still adds v.
+    static constexpr int TBL_PITCH = (F16 && Q <= 8) ? (1 << HB) + 4 : (1 << HB);     // q = 9: 256 x 260 would overflow the halfword
+    static constexpr int TBL_BYTES = NIBBLE ? (1 << SH) / 2 : (1 << HB) * TBL_PITCH;
+    static constexpr uint32_t VMASK = ((1u << HB) - 1u) << ISHIFT;      // the v bits of a column word
     static constexpr int TBL_AREA = (TBL_BYTES + 15) / 16 * 16;
     static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
     static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
@@ -596,7 +604,7 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
     const uint32_t w2mask = (y >= 2) ? FULL : 0u;
     const int c = B * Q + y;
     const int abot = A * Q + Q - 1;
-    const int shb = C::ISHIFT + HB + (y > 0 ? y - 1 : 0);   // position of my horizontal difference bit
+    const uint32_t khy = ((uint32_t)C::TBL_PITCH << (y > 0 ? y - 1 : 0)) << C::ISHIFT;   // index weight of my horizontal difference bit
     const int sh0 = C::ISHIFT + Q - 2 + y;                  // vertical bit of row x = s-y sits at sh0 - (s-1) (sh0 <= 31)
     const uint32_t XJ = MERGED ? 0u : sm.Xst[(ZOFF + B) * TP + c];
     uint32_t pms = 0;                                    // bit (x + y) <-> row x pairs with my column
@@ -653,7 +661,7 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         tR = tbl_gather<Q, true>(sm, tS);
         // ---- step a6, horizontal: my row word = neighbour's word | my difference bit
         const uint32_t vnew = tag_value<Q>(v);
-        const uint32_t wme = firstcol ? vnew : (Lw | ((uint32_t)(v - Lv) << shb));
+        const uint32_t wme = firstcol ? vnew : (Lw + (uint32_t)(v - Lv) * khy);
         if (live && lastcol) {
             wo[-s] = wme;
             if (DIAG) wo[-s + 8 * TP] = wme;
@@ -663,7 +671,7 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         // ---- step a6, vertical: the column word now starts at row a (anchor v, bit of the pair (a, a+1))
         {
             const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 1 ? s - 1 : 0) & 31);   // used for x >= 1 only
-            xbits = (y <= s - 1) ? ((xbits | dbit) & (C::IDXMASK << C::ISHIFT)) : 0u;     // x >= 1
+            xbits = (y <= s - 1) ? ((xbits | dbit) & C::VMASK) : 0u;     // x >= 1
             vsh = vnew;
         }
         if (x_lo >= 0 && live && y == x_lo) sm.Xst[A * TP + c] = xbits + vsh;    // x = Q-1: the column word is complete
@@ -1176,8 +1184,22 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, Cfg<Q>::MIN_CTAS) fill_kernel(Pa
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(p.tbl);
         uint4 *dst = reinterpret_cast<uint4 *>(sm.tbl);
-        for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
-        if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
+        if constexpr (C::TBL_PITCH == (1 << C::HB)) {
+            for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
+            if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
+        } else {
+            // padded pitch: row h of the compact table -> byte offset h * TBL_PITCH
+            constexpr int ROWB = 1 << C::HB;
+            if constexpr (ROWB % 4 == 0) {
+                const uint32_t *s32 = reinterpret_cast<const uint32_t *>(p.tbl);
+                for (int e = tid; e < ROWB * ROWB / 4; e += C::NTHR) {
+                    const int h = e / (ROWB / 4), w = e % (ROWB / 4);
+                    *reinterpret_cast<uint32_t *>(sm.tbl + h * C::TBL_PITCH + 4 * w) = __ldg(s32 + e);
+                }
+            } else {
+                for (int e = tid; e < ROWB * ROWB; e += C::NTHR) sm.tbl[(e / ROWB) * C::TBL_PITCH + e % ROWB] = p.tbl[e];
+            }
+        }
     }
     if (tid < C::MB_COUNT) {
         const int u = tid - C::MB_STEPIN;
