@@ -70,7 +70,9 @@ struct Cfg {
     static constexpr int RPT = Q;              // product phase: a thread owns RPT rows x 2 columns (c and c + T/2): the warp-uniform
     static constexpr int HT = T / 2;           // row words are loaded once for 2*RPT lookups (a broadcast LDS.128 costs 2 wavefronts)
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
-    static constexpr int VP = T + 1;           // pitch of the value array (int16): a wavefront step is conflict-free
+    static constexpr int VP = T + 10;          // pitch of the value arrays (int16) = 4q+5 words, odd and >= q/2 away from a multiple of 32:
+                                               // a column (lanes = rows), a q-tile patch (4 rows x q columns) and a skewed wavefront step
+                                               // (lane y on row a+y, column c+y) are all bank-conflict-free
     static constexpr int PANEL_WORDS = 8 * T;  // words in one row or column panel
     static constexpr int REC_BYTES = 2 * PANEL_WORDS * 4 + 2 * T * 2;   // PH, PV, top row, right column
     static constexpr int WROWS = 16;           // word-array rows: 8 groups of block I, 8 of block J
@@ -83,7 +85,7 @@ struct Cfg {
     static constexpr int VAL_ROWS = T + 1 + 2 * Q;   // Q guard rows, rows 0..T, Q guard rows
     static constexpr int VAL_BYTES = ((VAL_ROWS * VP + 2) * 2 + 15) / 16 * 16;
     static constexpr int STG_BYTES = 2 * 2 * PANEL_WORDS * 4;
-    static constexpr int VP2 = T + 2;          // pitch of val2 (int16): odd word stride, a column of it is conflict-free
+    static constexpr int VP2 = VP;             // pitch of val2 / val3
     static constexpr int VAL2_BYTES = (T * VP2 * 2 + 15) / 16 * 16;   // late products of block I+1 (kept apart: two warps merge concurrently)
     // closure warps: a warp runs G q-tiles of one anti-diagonal side by side (Q lanes each); NWV such warps cover
     // the <= 8 q-tiles of a macro-step; NMH helper warps prepare the next macro-step's older complete groups
