@@ -280,3 +280,57 @@ def test_determinism_repeat_calls(rna):
         b, tb = r.fold(s, table_dtype=rna.TABLE_INT16)
         torch.cuda.synchronize()
         assert int(a.item()) == int(b.item()) and torch.equal(ta, tb)
+
+
+# ------------------------------------------------------------------ pipelined closures, late products, q sweep
+@pytest.mark.parametrize("q", [5, 8, 9, 10])
+def test_midsize_scores_every_late_product_shape(rna, q):
+    """lengths of 2..9 super-tiles per side: super-tile diagonals dp = 1 (no late product), 2 (one block, both
+    operands arriving), 3 (two late blocks, no bulk stage) and >= 4 (bulk stages + late blocks); sampled cells
+    against the fast oracle"""
+    r = ctx(rna, q, rna.ENGINE_TILED)
+    T = 8 * q
+    rs = np.random.RandomState(4000 + q)
+    for nt in (2, 3, 4, 5, 7, 9):
+        n = nt * T - int(rs.randint(0, T))
+        s = rand_seq(rs, n)
+        cells = np.stack([rs.randint(1, n + 1, size=400), rs.randint(1, n + 1, size=400)], axis=1).astype(np.int32)
+        cells.sort(axis=1)
+        want = oracle.nussinov_fast(s, threads=4, cells=cells)
+        score, tab = r.fold(dev_seq(s), table_dtype=rna.TABLE_INT16)
+        torch.cuda.synchronize()
+        assert int(score.item()) == want["score"], (q, n)
+        got = tab.cpu().numpy()[cells[:, 0] - 1, cells[:, 1] - 1]
+        assert (got == want["cells"]).all(), (q, n)
+
+
+def test_skewed_base_distributions(rna):
+    """long runs of equal difference vectors (all-zero, all-one) and rare pairs: sequences far from uniform"""
+    r = ctx(rna, 8, rna.ENGINE_TILED)
+    rs = np.random.RandomState(77)
+    for p in ([0.97, 0.01, 0.01, 0.01], [0.49, 0.01, 0.01, 0.49], [0.05, 0.45, 0.45, 0.05], [0.7, 0.0, 0.0, 0.3]):
+        n = int(rs.randint(500, 900))
+        s = bytes(rs.choice(list(b"ACGU"), size=n, p=p).tolist())
+        want_score, want = oracle.nussinov(s, want_table=True)
+        got_score, got = gpu_table(rna, r, s, rna.TABLE_INT16)
+        assert got_score == want_score and (got.astype(np.int32) == want).all(), p
+
+
+@pytest.mark.parametrize("q", [4, 9, 10])
+def test_batch_other_q(rna, q):
+    r = ctx(rna, q, rna.ENGINE_TILED)
+    seqs, _ = workloads.random_sequences(500 + q, 40, 0, 450)
+    flat, offsets, lens = workloads.pack_batch(seqs)
+    got = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens)
+    torch.cuda.synchronize()
+    assert (got.cpu().numpy() == np.array([oracle.nussinov(x) for x in seqs])).all()
+
+
+def test_length_limit_of_the_word_format(rna):
+    """q = 10 keeps 14 value bits above its 18 index bits: n <= 2 * (2^14 - 1 - q); q <= 9 takes the ABI's 65534"""
+    r10 = ctx(rna, 10, rna.ENGINE_TILED)
+    lim = 2 * ((1 << 14) - 1 - 10)
+    assert r10.workspace_bytes(lim) > 0
+    with pytest.raises(rna.Rna4rError) as e:
+        r10.fold(dev_seq(b"A" * 16), n=lim + 1, workspace=torch.empty(1 << 20, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == -3
