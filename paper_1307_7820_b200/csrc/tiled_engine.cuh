@@ -65,7 +65,7 @@ struct Cfg {
     static constexpr int TBL_AREA = (TBL_BYTES + 15) / 16 * 16;
     static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
     static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
-    static constexpr int NTHR = WTHR + 128;    // + 4 helper warps of the closure: loader, publisher, 2 x late products
+    static constexpr int NTHR = WTHR + 128;    // + 4 warps: a closure needs NROLE = NWV + NMH + 8 warps
     static constexpr int MIN_CTAS = (Q <= 8) ? 3 : 1;   // register budget: 3 CTAs per SM while the table is small
     static constexpr int RPT = Q;              // product phase: a thread owns RPT rows x 2 columns (c and c + T/2): the warp-uniform
     static constexpr int HT = T / 2;           // row words are loaded once for 2*RPT lookups (a broadcast LDS.128 costs 2 wavefronts)
