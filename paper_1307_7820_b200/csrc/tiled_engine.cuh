@@ -705,11 +705,7 @@ struct CloseCtx {
 __device__ __forceinline__ void warp_wait_flag_ge(const int *flag, int v, int lane)
 {
     if (lane == 0) {
-        if (ld_acquire_gpu(flag) < v) {
-            unsigned ns = 32;
-            while (ld_relaxed_gpu(flag) < v) { __nanosleep(ns); if (ns < 256) ns *= 2; }
-            (void)ld_acquire_gpu(flag);
-        }
+        while (ld_acquire_gpu(flag) < v) __nanosleep(32);     // every poll is an acquire: no second round trip once the flag is seen
     }
     __syncwarp();
 }
