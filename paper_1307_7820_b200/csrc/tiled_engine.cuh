@@ -99,8 +99,9 @@ struct Cfg {
     // from the late-product helpers has been merged: the left (right) half of q-row A's late products arrives at
     // u = 7-A (11-A), the lower (upper) half of q-column B's at u = B (B+4) -- see stepin_count()
     static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_STEPIN = 32, MB_COUNT = 48;
+    static constexpr int MB_PROD = 48, MB_TOTAL = 52;    // bulk product: operands landed [48,50), buffer free [50,52)
     __host__ __device__ static constexpr int stepin_count(int u) { return (u <= 3) ? 2 : (u <= 7) ? 4 : (u <= 11) ? 2 : 0; }
-    static constexpr int MBAR_BYTES = MB_COUNT * 8;
+    static constexpr int MBAR_BYTES = MB_TOTAL * 8;
     static_assert(NROLE * 32 <= NTHR, "closure roles must fit the CTA");
     static constexpr int POST_BYTES = VAL_BYTES + 2 * VAL2_BYTES + STG_BYTES + ((2 * T + 15) / 16 * 16) + 64 + MBAR_BYTES;
     // The table sits at the START of the dynamic window.  F16: the gather address is (S >> 16) + base with no
@@ -419,6 +420,43 @@ __device__ __forceinline__ void product_accumulate(const Smem<Q> &sm, int buf, u
     }
 }
 
+// ---- mbarrier / bulk-copy primitives ----
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.release.cta.shared.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.acquire.cta.shared.b64 P1, [%0], %1, %2;\n"
+        "@P1 bra.uni WAIT_DONE;\n"
+        "bra.uni WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_addr(bar)), "r"(parity), "r"(20000u) : "memory");     // suspend-time hint (ns): park, do not spin
+}
+
+__device__ __forceinline__ void mbar_inval(uint64_t *bar)
+{
+    asm volatile("mbarrier.inval.shared.b64 [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+// TMA 1-D bulk copy global -> shared; completion is signalled on `bar` (complete_tx)
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_addr(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+
 // ---- PROD task: merge the products of newly available middle blocks into the target's acc ----
 template <int Q>
 __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, int I, int J, int s)
@@ -439,37 +477,59 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 
     // K sequence: for m = lo..hi: K = I+m, then K = J-m (if different)
     const int nk_max = 2 * (hi - lo + 1);
-    int issued = 0, computed = 0;
     auto kth = [&](int e) -> int {           // e-th block of the sequence, or -1 for the duplicate
         const int m = lo + (e >> 1);
         const int K = (e & 1) ? (J - m) : (I + m);
         if ((e & 1) && (J - m == I + m)) return -1;
         return K;
     };
-    // software pipeline: operands of element e+1 are in flight while element e is computed
-    int e_next = 0;
-    auto issue_next = [&]() -> bool {
-        while (e_next < nk_max) {
-            const int K = kth(e_next++);
-            if (K < 0) continue;
-            const int s_ik = si.sbase + tri_index(nt, I, K), s_kj = si.sbase + tri_index(nt, K, J);
-            if (tid == 0) { wait_flag_ge(p.done + s_ik, 1); wait_flag_ge(p.done + s_kj, 1); }
-            __syncthreads();
-            load_operands_async<Q>(p, sm, issued & 1, s_ik, s_kj);
-            ++issued;
-            return true;
+    // Warp-specialised operand pipeline: one producer warp (the first warp beyond the product threads) waits for
+    // the operand tiles' flags and fetches PH(I,K), PV(K,J) with two TMA bulk copies per block into a two-deep
+    // ring; the product warps only ever wait on the ring's mbarriers, so flag and L2 latency stay off their path.
+    constexpr int NPW = C::PTHR / 32;                      // product warps
+    constexpr uint32_t PANEL_BYTES = C::PANEL_WORDS * 4;
+    uint64_t *full = sm.mbar + C::MB_PROD, *empty = full + 2;
+    if (tid == 0) {
+        for (int b = 0; b < 2; ++b) {
+            mbar_inval(full + b); mbar_inval(empty + b);
+            mbar_init(full + b, 1); mbar_init(empty + b, NPW);
         }
-        return false;
-    };
-    issue_next();
-    while (computed < issued) {
-        const bool more = issue_next();
-        if (more) cp_async_wait<1>(); else cp_async_wait<0>();
-        __syncthreads();
-        if (pact) product_accumulate<Q>(sm, computed & 1, acc, cj, rb);
-        ++computed;
-        __syncthreads();     // the buffer may be refilled by the next issue
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
+    __syncthreads();
+    const int warp = tid >> 5, lane = tid & 31;
+    if (warp == NPW) {
+        if (lane == 0) {
+            int i = 0;
+            for (int e = 0; e < nk_max; ++e) {
+                const int K = kth(e);
+                if (K < 0) continue;
+                const int b = i & 1, k = i >> 1;
+                if (k >= 1) mbar_wait(empty + b, (uint32_t)(k - 1) & 1u);       // the product warps are done with the buffer
+                const int s_ik = si.sbase + tri_index(nt, I, K), s_kj = si.sbase + tri_index(nt, K, J);
+                wait_flag_ge(p.done + s_ik, 1);
+                wait_flag_ge(p.done + s_kj, 1);
+                uint32_t *dst = sm.stg + (size_t)b * 2 * C::PANEL_WORDS;
+                mbar_expect_tx(full + b, 2 * PANEL_BYTES);
+                bulk_g2s(dst, rec_ptr<Q>(p, s_ik), PANEL_BYTES, full + b);                                   // PH of (I,K)
+                bulk_g2s(dst + C::PANEL_WORDS, rec_ptr<Q>(p, s_kj) + PANEL_BYTES, PANEL_BYTES, full + b);     // PV of (K,J)
+                ++i;
+            }
+        }
+    } else if (pact) {
+        int i = 0;
+        for (int e = 0; e < nk_max; ++e) {
+            if (kth(e) < 0) continue;
+            const int b = i & 1, k = i >> 1;
+            mbar_wait(full + b, (uint32_t)k & 1u);
+            product_accumulate<Q>(sm, b, acc, cj, rb);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + b);
+            ++i;
+        }
+    }
+    __syncthreads();
     // merge with earlier stages (they ran at earlier steps and own acc until their release)
     int16_t *accg = p.acc + (size_t)sidx * C::T * C::T;
     if (s != S - 1) {
@@ -528,26 +588,6 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
 // DIAG (I == J): row and column words are both the tile's own (z < 8 only); macro-steps start at u = 7;
 // in q-tile (B,B) head and tail are ONE lookup (row word through c-2, Xp); cells with c-a <= 1 are 0.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.release.cta.shared.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.acquire.cta.shared.b64 P1, [%0], %1, %2;\n"
-        "@P1 bra.uni WAIT_DONE;\n"
-        "bra.uni WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_addr(bar)), "r"(parity), "r"(20000u) : "memory");     // suspend-time hint (ns): park, do not spin
-}
 
 // Complete-group lookups for the Q x Q cells of q-tile (A,B), all 32 lanes: for z in [zlo, zhi],
 // val[a][c] = max(val[a][c], lookup(W[z*wp + a] + X[z*xp + c])).  Used for the mini-products of the
