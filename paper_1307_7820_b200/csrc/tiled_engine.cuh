@@ -84,7 +84,8 @@ struct Cfg {
     static constexpr int PRE_BYTES = (W_GUARD + 2 * W_BYTES + 15) / 16 * 16;
     static constexpr int VAL_ROWS = T + 1 + 2 * Q;   // Q guard rows, rows 0..T, Q guard rows
     static constexpr int VAL_BYTES = ((VAL_ROWS * VP + 2) * 2 + 15) / 16 * 16;
-    static constexpr int STG_BYTES = 2 * 2 * PANEL_WORDS * 4;
+    static constexpr int NSTG = 2;             // depth of the bulk product's operand ring
+    static constexpr int STG_BYTES = NSTG * 2 * PANEL_WORDS * 4;
     static constexpr int VP2 = VP;             // pitch of val2 / val3
     static constexpr int VAL2_BYTES = (T * VP2 * 2 + 15) / 16 * 16;   // late products of block I+1 (kept apart: two warps merge concurrently)
     // closure warps: a warp runs G q-tiles of one anti-diagonal side by side (Q lanes each); NWV such warps cover
@@ -99,7 +100,7 @@ struct Cfg {
     // from the late-product helpers has been merged: the left (right) half of q-row A's late products arrives at
     // u = 7-A (11-A), the lower (upper) half of q-column B's at u = B (B+4) -- see stepin_count()
     static constexpr int MB_STEP = 0, MB_ROW = 16, MB_COL = 24, MB_STEPIN = 32, MB_COUNT = 48;
-    static constexpr int MB_PROD = 48, MB_TOTAL = 52;    // bulk product: operands landed [48,50), buffer free [50,52)
+    static constexpr int MB_PROD = 48, MB_TOTAL = 56;    // bulk product ring: operands landed [48,48+NSTG), buffer free [52,52+NSTG)
     __host__ __device__ static constexpr int stepin_count(int u) { return (u <= 3) ? 2 : (u <= 7) ? 4 : (u <= 11) ? 2 : 0; }
     static constexpr int MBAR_BYTES = MB_TOTAL * 8;
     static_assert(NROLE * 32 <= NTHR, "closure roles must fit the CTA");
@@ -484,16 +485,18 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
         return K;
     };
     // Warp-specialised operand pipeline: one producer warp (the first warp beyond the product threads) waits for
-    // the operand tiles' flags and fetches PH(I,K), PV(K,J) with two TMA bulk copies per block into a two-deep
+    // the operand tiles' flags and fetches PH(I,K), PV(K,J) with two TMA bulk copies per block into a NSTG-deep
     // ring; the product warps only ever wait on the ring's mbarriers, so flag and L2 latency stay off their path.
     constexpr int NPW = C::PTHR / 32;                      // product warps
     constexpr uint32_t PANEL_BYTES = C::PANEL_WORDS * 4;
-    uint64_t *full = sm.mbar + C::MB_PROD, *empty = full + 2;
+    constexpr int NSTG = C::NSTG;
+    uint64_t *full = sm.mbar + C::MB_PROD, *empty = full + 4;
     if (tid == 0) {
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < NSTG; ++b) {
             mbar_inval(full + b); mbar_inval(empty + b);
             mbar_init(full + b, 1); mbar_init(empty + b, NPW);
         }
+        mbar_inval(full + 3); mbar_init(full + 3, 1);          // the acc tile of the earlier stages has landed
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -505,7 +508,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
             for (int e = 0; e < nk_max; ++e) {
                 const int K = kth(e);
                 if (K < 0) continue;
-                const int b = i & 1, k = i >> 1;
+                const int b = i % NSTG, k = i / NSTG;
                 if (k >= 1) mbar_wait(empty + b, (uint32_t)(k - 1) & 1u);       // the product warps are done with the buffer
                 const int s_ik = si.sbase + tri_index(nt, I, K), s_kj = si.sbase + tri_index(nt, K, J);
                 wait_flag_ge(p.done + s_ik, 1);
@@ -516,34 +519,35 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
                 bulk_g2s(dst + C::PANEL_WORDS, rec_ptr<Q>(p, s_kj) + PANEL_BYTES, PANEL_BYTES, full + b);     // PV of (K,J)
                 ++i;
             }
+            if (s != S - 1) {
+                // earlier stages (they ran at earlier steps and own acc until their release): fetch their maxima
+                wait_flag_ge(p.accstage + sidx, S - 1 - s);
+                mbar_expect_tx(full + 3, (uint32_t)(C::T * C::T * 2));
+                bulk_g2s(sm.valraw, p.acc + (size_t)sidx * C::T * C::T, (uint32_t)(C::T * C::T * 2), full + 3);
+            }
         }
     } else if (pact) {
         int i = 0;
         for (int e = 0; e < nk_max; ++e) {
             if (kth(e) < 0) continue;
-            const int b = i & 1, k = i >> 1;
+            const int b = i % NSTG, k = i / NSTG;
             mbar_wait(full + b, (uint32_t)k & 1u);
             product_accumulate<Q>(sm, b, acc, cj, rb);
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + b);
             ++i;
         }
-    }
-    __syncthreads();
-    // merge with earlier stages (they ran at earlier steps and own acc until their release)
-    int16_t *accg = p.acc + (size_t)sidx * C::T * C::T;
-    if (s != S - 1) {
-        if (tid == 0) wait_flag_ge(p.accstage + sidx, S - 1 - s);
-        __syncthreads();
-        if (pact) {
+        if (s != S - 1) {
+            mbar_wait(full + 3, 0u);
 #pragma unroll
             for (int rr = 0; rr < C::RPT; ++rr) {
-                const int16_t *row = accg + (size_t)(rb * C::RPT + rr) * C::T + cj;
-                acc[0][rr] = tag_max<Q>(acc[0][rr], tag_value<Q>((int)__ldcg(row)));
-                acc[1][rr] = tag_max<Q>(acc[1][rr], tag_value<Q>((int)__ldcg(row + C::HT)));
+                const int16_t *row = sm.valraw + (rb * C::RPT + rr) * C::T + cj;
+                acc[0][rr] = tag_max<Q>(acc[0][rr], tag_value<Q>((int)row[0]));
+                acc[1][rr] = tag_max<Q>(acc[1][rr], tag_value<Q>((int)row[C::HT]));
             }
         }
     }
+    int16_t *accg = p.acc + (size_t)sidx * C::T * C::T;
     if (pact) {
 #pragma unroll
         for (int rr = 0; rr < C::RPT; ++rr) {
