@@ -556,7 +556,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
             __stcg(row + C::HT, (int16_t)untag<Q>(acc[1][rr]));
         }
     }
-    __threadfence();
+    // the CTA barrier orders every thread's stores before thread 0's release (cumulative): no per-thread fence
     __syncthreads();
     if (tid == 0) st_release_gpu(p.accstage + sidx, S - s);
 }
@@ -1203,8 +1203,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
         }
         if (I == 0 && J == n / T && tid == 0)
             p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
-        __threadfence();
-        __syncthreads();
+        __syncthreads();               // orders every thread's stores before thread 0's releases (cumulative)
         if (tid == 0) {
             if (dp == 0) { st_release_gpu(cc.rowprogX, 8); st_release_gpu(cc.colprogX, 8); }
             st_release_gpu(p.done + sidx, 1);
