@@ -337,15 +337,6 @@ __device__ __forceinline__ uint32_t lookup_max(const Smem<Q> &sm, uint32_t S, ui
     else return max(acc, S + (rv << Cfg<Q>::SH));
 }
 
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
-{
-    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 // Polls are relaxed loads (an acquire load also invalidates the L1 on every iteration); one acquire load
 // orders the data reads after the flag has been seen.
 __device__ __forceinline__ int ld_relaxed_gpu(const int *p)
@@ -364,23 +355,6 @@ __device__ __forceinline__ void wait_flag_ge(const int *flag, int v)
 
 template <int Q>
 __device__ __forceinline__ const uint8_t *rec_ptr(const Params &p, int sidx) { return p.recs + (size_t)sidx * Cfg<Q>::REC_BYTES; }
-
-// issue the async copy of PH(I,K) and PV(K,J) into stage buffer `buf` (one 16-byte chunk per thread)
-template <int Q>
-__device__ __forceinline__ void load_operands_async(const Params &p, const Smem<Q> &sm, int buf, int sidx_ik, int sidx_kj)
-{
-    using C = Cfg<Q>;
-    const int tid = threadIdx.x;
-    constexpr int CH = C::PANEL_WORDS / 4;        // 16-byte chunks per panel = 2T
-    uint32_t *dst = sm.stg + (size_t)buf * 2 * C::PANEL_WORDS;
-    if (tid < CH) {
-        cp_async16(dst + tid * 4, rec_ptr<Q>(p, sidx_ik) + (size_t)tid * 16);                               // PH of (I,K)
-    } else if (tid < 2 * CH) {
-        const int c = tid - CH;
-        cp_async16(dst + C::PANEL_WORDS + c * 4, rec_ptr<Q>(p, sidx_kj) + (size_t)C::PANEL_WORDS * 4 + (size_t)c * 16);   // PV of (K,J)
-    }
-    cp_async_commit();
-}
 
 // bulk step (a4): acc[h][rr] = max over the 8 groups of block K, for columns cj + h*T/2 and rows rb*RPT+rr.
 // acc is kept in the tagged form (value field + don't-care index bits); tag_max orders by value.
@@ -601,7 +575,7 @@ __device__ __forceinline__ void qtile_groups(const Smem<Q> &sm, int A, int B, co
                                              int zlo, int zhi, int lane, bool merge2 = false, bool out3 = false)
 {
     using C = Cfg<Q>;
-    constexpr int VP = C::VP, SH = C::SH;
+    constexpr int VP = C::VP;
     constexpr int RS = (32 / Q > Q) ? Q : 32 / Q;        // row slots
     constexpr int NX = (Q + RS - 1) / RS;                // rows per lane
     const int my = lane % Q, xr = lane / Q;
@@ -641,7 +615,7 @@ template <int Q, bool DIAG, bool MERGED>
 __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int lane, bool own)
 {
     using C = Cfg<Q>;
-    constexpr int TP = C::TP, VP = C::VP, SH = C::SH, HB = C::HB;
+    constexpr int TP = C::TP, VP = C::VP, SH = C::SH;
     constexpr uint32_t FULL = 0xffffffffu;
     constexpr int ZOFF = DIAG ? 0 : 8;
     const int y = lane % Q;                              // lane group lane/Q runs q-tile (A,B); !own: shadow, stores nothing
@@ -777,7 +751,7 @@ template <int Q, bool DIAG>
 __device__ __forceinline__ void qtile_fresh_merge(const Smem<Q> &sm, int A, int B, int lane, bool use2)
 {
     using C = Cfg<Q>;
-    constexpr int TP = C::TP, VP = C::VP, VP2 = C::VP2, SH = C::SH;
+    constexpr int TP = C::TP, VP = C::VP, VP2 = C::VP2;
     constexpr int ZOFF = DIAG ? 0 : 8;
     constexpr int RS = (32 / Q > Q) ? Q : 32 / Q;        // row slots
     constexpr int NX = (Q + RS - 1) / RS;                // rows per lane
@@ -1003,7 +977,7 @@ __device__ __forceinline__ void late_strip(const Smem<Q> &sm, const uint32_t *U,
 {
     // U[g*T + u0 + i], i < Q: the uniform side; L[g*T + l], l0 <= l < l1: the lane side; out[(u0+i)*out_us + l*out_ls]
     using C = Cfg<Q>;
-    constexpr int T = C::T, SH = C::SH;
+    constexpr int T = C::T;
     for (int l = l0 + lane; l < l1; l += 32) {
         uint32_t acc[Q];
 #pragma unroll
