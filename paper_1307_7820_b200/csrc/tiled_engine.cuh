@@ -1332,11 +1332,8 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     p.scores = scores; p.table_out = table_out; p.table_dtype = table_dtype;
     p.trace = ctx->trace; p.trace_tiles = ctx->trace_tiles;
 
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (ctx->tiled_blocks_per_sm == 0)     // first launch of this context (one q, one device): opt in to the large shared window
         RNA4R_CUDA(ctx, cudaFuncSetAttribute(fill_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-        attr_set = true;
-    }
     if (ctx->tiled_blocks_per_sm == 0) {
         int nb = 0;
         RNA4R_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fill_kernel<Q>, C::NTHR, C::SMEM_BYTES));
