@@ -1353,9 +1353,9 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     size_t want = h.tasks;
     int per_sm = ctx->tiled_blocks_per_sm;
     // A single fold of moderate length is bound by the closure chain, and a closure runs faster with fewer
-    // neighbours on its SM (measured at n=6000: 2.30 ms with 2 CTAs/SM, 2.41 ms with 3); long folds and batches are
-    // throughput-bound and take every CTA they can get (n=16384: 22.4 ms with 3, 25 ms with 2).
-    if (count == 1 && h.max_nt <= 128 && per_sm > 2) per_sm = 2;
+    // neighbours on its SM (measured at n=6000: 1.98 ms with 2 CTAs/SM, 2.11 ms with 3; n=2000: 0.60 / 0.64); long folds and
+    // batches are throughput-bound and take every CTA they can get (n=8000: 3.43 ms with 3, 3.48 with 2; n=16384: 18.8 / 21).
+    if (count == 1 && h.max_nt <= 112 && per_sm > 2) per_sm = 2;
     if (const char *e = getenv("RNA4R_BLOCKS_PER_SM")) { const int v = atoi(e); if (v >= 1 && v < per_sm) per_sm = v; }   // tuning knob
     int blocks = ctx->sm_count * per_sm;
     if ((size_t)blocks > want) blocks = (int)want;
