@@ -656,10 +656,7 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         const uint32_t w_cur = w_nxt;
         const int o_cur = o_nxt, lv_cur = lv_nxt;
         if (s < 2 * Q - 2) { w_nxt = wb[-(s + 1)]; o_nxt = vb[-(s + 2) * VP]; lv_nxt = vb[-(s + 1) * VP - 1]; }
-        // ---- oldx of my cell: fold in the lookups issued in the previous step
-        uint32_t best = 0;
-        if (!MERGED) best = Cfg<Q>::F16 ? __viaddmax_u16x2(hS, hR, 0u) : hS + (hR << SH);
-        best = Cfg<Q>::F16 ? __viaddmax_u16x2(tS, tR, best) : max(best, tS + (tR << SH));
+        const uint32_t phS = hS, phR = hR, ptS = tS, ptR = tR;      // the lookups issued in the previous step (my cell's)
         // ---- head lookup of the NEXT cell: running column word (rows >= a+1) x row word of group A of block I
         uint32_t Xp = xbits + vsh;
         if (s + 1 < Q && y > s) Xp = 0;                             // not in the q-tile yet: no row of it lies below
@@ -670,8 +667,13 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         const uint32_t Lw2 = __shfl_sync(FULL, wout, src2) & w2mask;   // row a-1 through column c-2
         if (firstcol) Lv = lv_cur;                                  // column c-1 belongs to the q-tile on the left
         // ---- the cell (a3 init + a5 fresh splits)
-        const int oldx = max(o_pend, untag<Q>(best));
-        int v = max(max(oldx, vprev), Lv);
+        // The pending lookups are folded in with the direct candidates as their accumulator: their consumers then
+        // depend on the shuffle result and cannot be scheduled -- with their wait for the gathers -- before the
+        // shuffles are issued (a single warp issues in order).
+        uint32_t best = tag_value<Q>(max(max(o_pend, vprev), Lv));
+        if (!MERGED) best = Cfg<Q>::F16 ? __viaddmax_u16x2(phS, phR, best) : max(best, phS + (phR << SH));
+        best = Cfg<Q>::F16 ? __viaddmax_u16x2(ptS, ptR, best) : max(best, ptS + (ptR << SH));
+        int v = untag<Q>(best);
         if (s + 1 < Q && y == s + 1) v = vbelow;                    // pre-step (x = -1): the cell below the q-tile
         if (MERGED && s - (Q - 1) <= 1) v = 0;                      // D(i,i) = D(i,i-1) = 0
         const bool live = own && (unsigned)(s - y) < (unsigned)Q;
@@ -720,12 +722,15 @@ struct CloseCtx {
 };
 #define RNA4R_EV(cc, idx) do { if (RNA4R_TRACE_WORDS > 8 && (cc).ev && lane == 0) (cc).ev[idx] = global_timer_ns(); } while (0)
 
-__device__ __forceinline__ void warp_wait_flag_ge(const int *flag, int v, int lane)
+// waits until *flag >= v; returns the value seen (clamped to 8: the flags count q-rows / q-columns)
+__device__ __forceinline__ int warp_wait_flag_ge(const int *flag, int v, int lane)
 {
+    int have = 0;
     if (lane == 0) {
-        while (ld_acquire_gpu(flag) < v) __nanosleep(32);     // every poll is an acquire: no second round trip once the flag is seen
+        while ((have = ld_acquire_gpu(flag)) < v) __nanosleep(32);     // every poll is an acquire: no second round trip once the flag is seen
     }
-    __syncwarp();
+    have = __shfl_sync(0xffffffffu, have, 0);
+    return have < 8 ? have : 8;
 }
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
@@ -893,16 +898,22 @@ __device__ __forceinline__ void close_col_loader(const Smem<Q> &sm, const CloseC
         }
         sm.val[T * VP] = (int16_t)corner;
     }
-    for (int B = 0; B < 8; ++B) {
-        warp_wait_flag_ge(cc.colprogY, B + 1, lane);
-        for (int e = lane; e < 8 * Q; e += 32) {
-            const int g = e / Q, k = B * Q + e % Q;
-            YX[g * T + k] = __ldcg(pv + g * T + k);
+    int loaded = 0;
+    while (loaded < 8) {
+        const int have = min(warp_wait_flag_ge(cc.colprogY, loaded + 1, lane), loaded + 2);
+        for (int B = loaded; B < have; ++B) {
+            for (int e = lane; e < 8 * Q; e += 32) {
+                const int g = e / Q, k = B * Q + e % Q;
+                YX[g * T + k] = __ldcg(pv + g * T + k);
+            }
+            if (lane < Q) sm.val[T * VP + B * Q + lane + 1] = (int16_t)__ldcg(etop + B * Q + lane);
         }
-        if (lane < Q) sm.val[T * VP + B * Q + lane + 1] = (int16_t)__ldcg(etop + B * Q + lane);
         __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + C::MB_COL + B);
-        RNA4R_EV(cc, 144 + B);
+        for (int B = loaded; B < have; ++B) {
+            if (lane == 0) mbar_arrive(sm.mbar + C::MB_COL + B);
+            RNA4R_EV(cc, 144 + B);
+        }
+        loaded = have;
     }
 }
 
@@ -916,16 +927,24 @@ __device__ __forceinline__ void close_row_loader(const Smem<Q> &sm, const CloseC
     const uint32_t *ph = reinterpret_cast<const uint32_t *>(cc.recZ);
     const uint16_t *eright = reinterpret_cast<const uint16_t *>(cc.recZ + 2 * C::PANEL_WORDS * 4) + T;
     uint32_t *ZW = panel_ZW<Q>(sm);
-    for (int A = 7; A >= 0; --A) {
-        warp_wait_flag_ge(cc.rowprogZ, 8 - A, lane);
-        for (int e = lane; e < 8 * Q; e += 32) {
-            const int g = e / Q, k = A * Q + e % Q;
-            ZW[g * T + k] = __ldcg(ph + g * T + k);
+    // One iteration costs two dependent L2 round trips (flag, data): when the neighbour is ahead, every q-row it
+    // has published is fetched in the same iteration, so the loader never falls behind the neighbour's pace.
+    int loaded = 0;
+    while (loaded < 8) {
+        const int have = min(warp_wait_flag_ge(cc.rowprogZ, loaded + 1, lane), loaded + 2);   // at most 2 per iteration: the first one is urgent
+        for (int A = 7 - loaded; A >= 8 - have; --A) {
+            for (int e = lane; e < 8 * Q; e += 32) {
+                const int g = e / Q, k = A * Q + e % Q;
+                ZW[g * T + k] = __ldcg(ph + g * T + k);
+            }
+            if (lane < Q) sm.val[(A * Q + lane) * VP] = (int16_t)__ldcg(eright + A * Q + lane);
         }
-        if (lane < Q) sm.val[(A * Q + lane) * VP] = (int16_t)__ldcg(eright + A * Q + lane);
         __syncwarp();
-        if (lane == 0) mbar_arrive(sm.mbar + C::MB_ROW + A);
-        RNA4R_EV(cc, 136 + A);
+        for (int A = 7 - loaded; A >= 8 - have; --A) {
+            if (lane == 0) mbar_arrive(sm.mbar + C::MB_ROW + A);
+            RNA4R_EV(cc, 136 + A);
+        }
+        loaded = have;
     }
 }
 
