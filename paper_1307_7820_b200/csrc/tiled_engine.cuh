@@ -879,6 +879,60 @@ __device__ __forceinline__ void close_mini_helper(const Smem<Q> &sm, const Close
     }
 }
 
+// Loader loop shared by the row and the column loader.  `unit` counts q-rows from the bottom (q-columns from the
+// left) in publishing order; unit k covers words [g][first(k) .. first(k)+Q) of the neighbour's panel `src` (pitch
+// T) and Q edge values.  Up to two published units are fetched per iteration, and the next flag read is issued
+// while their data is still in flight, so an iteration costs one L2 round trip instead of two.
+template <int Q, typename FirstOf, typename EdgeDst>
+__device__ __forceinline__ void loader_loop(const int *flag, const uint32_t *src, const uint16_t *esrc, uint32_t *dst, FirstOf first_of,
+                                            EdgeDst edge_dst, uint64_t *bars, const CloseCtx &cc, int ev0, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr int T = C::T;
+    constexpr int NW = (8 * Q + 31) / 32;
+    int have = warp_wait_flag_ge(flag, 1, lane);
+    int loaded = 0;
+    while (loaded < 8) {
+        const int hi = min(have, loaded + 2);
+        uint32_t w[2][NW];
+        uint16_t ev[2];
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const int k0 = first_of(min(loaded + r, 7));
+#pragma unroll
+            for (int i = 0; i < NW; ++i) {
+                const int e = lane + 32 * i;
+                w[r][i] = (e < 8 * Q && loaded + r < hi) ? __ldcg(src + (e / Q) * T + k0 + e % Q) : 0u;
+            }
+            ev[r] = (lane < Q && loaded + r < hi) ? __ldcg(esrc + k0 + lane) : (uint16_t)0;
+        }
+        int next = 8;
+        if (hi < 8 && lane == 0) next = ld_acquire_gpu(flag);         // in flight together with the data
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            if (loaded + r < hi) {
+                const int k0 = first_of(loaded + r);
+#pragma unroll
+                for (int i = 0; i < NW; ++i) {
+                    const int e = lane + 32 * i;
+                    if (e < 8 * Q) dst[(e / Q) * T + k0 + e % Q] = w[r][i];
+                }
+                if (lane < Q) *edge_dst(k0 + lane) = (int16_t)ev[r];
+            }
+        }
+        __syncwarp();
+        for (int k = loaded; k < hi; ++k) {
+            if (lane == 0) mbar_arrive(bars + first_of(k) / Q);
+            RNA4R_EV(cc, ev0 + first_of(k) / Q);
+        }
+        loaded = hi;
+        if (loaded < 8) {
+            have = min(__shfl_sync(0xffffffffu, next, 0), 8);
+            if (have <= loaded) have = warp_wait_flag_ge(flag, loaded + 1, lane);
+        }
+    }
+}
+
 // helper warp: columns of the tile below, q-column by q-column as it publishes them (column words for the
 // late products, top-row values = my bottom edge), and the corner value
 template <int Q>
@@ -898,23 +952,8 @@ __device__ __forceinline__ void close_col_loader(const Smem<Q> &sm, const CloseC
         }
         sm.val[T * VP] = (int16_t)corner;
     }
-    int loaded = 0;
-    while (loaded < 8) {
-        const int have = min(warp_wait_flag_ge(cc.colprogY, loaded + 1, lane), loaded + 2);
-        for (int B = loaded; B < have; ++B) {
-            for (int e = lane; e < 8 * Q; e += 32) {
-                const int g = e / Q, k = B * Q + e % Q;
-                YX[g * T + k] = __ldcg(pv + g * T + k);
-            }
-            if (lane < Q) sm.val[T * VP + B * Q + lane + 1] = (int16_t)__ldcg(etop + B * Q + lane);
-        }
-        __syncwarp();
-        for (int B = loaded; B < have; ++B) {
-            if (lane == 0) mbar_arrive(sm.mbar + C::MB_COL + B);
-            RNA4R_EV(cc, 144 + B);
-        }
-        loaded = have;
-    }
+    loader_loop<Q>(cc.colprogY, pv, etop, YX, [](int k) { return k * Q; },
+                   [&](int c) { return sm.val + T * VP + c + 1; }, sm.mbar + C::MB_COL, cc, 144, lane);
 }
 
 // helper warp: rows of the left tile, q-row by q-row as it publishes them (row words for the late
@@ -927,25 +966,8 @@ __device__ __forceinline__ void close_row_loader(const Smem<Q> &sm, const CloseC
     const uint32_t *ph = reinterpret_cast<const uint32_t *>(cc.recZ);
     const uint16_t *eright = reinterpret_cast<const uint16_t *>(cc.recZ + 2 * C::PANEL_WORDS * 4) + T;
     uint32_t *ZW = panel_ZW<Q>(sm);
-    // One iteration costs two dependent L2 round trips (flag, data): when the neighbour is ahead, every q-row it
-    // has published is fetched in the same iteration, so the loader never falls behind the neighbour's pace.
-    int loaded = 0;
-    while (loaded < 8) {
-        const int have = min(warp_wait_flag_ge(cc.rowprogZ, loaded + 1, lane), loaded + 2);   // at most 2 per iteration: the first one is urgent
-        for (int A = 7 - loaded; A >= 8 - have; --A) {
-            for (int e = lane; e < 8 * Q; e += 32) {
-                const int g = e / Q, k = A * Q + e % Q;
-                ZW[g * T + k] = __ldcg(ph + g * T + k);
-            }
-            if (lane < Q) sm.val[(A * Q + lane) * VP] = (int16_t)__ldcg(eright + A * Q + lane);
-        }
-        __syncwarp();
-        for (int A = 7 - loaded; A >= 8 - have; --A) {
-            if (lane == 0) mbar_arrive(sm.mbar + C::MB_ROW + A);
-            RNA4R_EV(cc, 136 + A);
-        }
-        loaded = have;
-    }
+    loader_loop<Q>(cc.rowprogZ, ph, eright, ZW, [](int k) { return (7 - k) * Q; },
+                   [&](int a) { return sm.val + a * VP; }, sm.mbar + C::MB_ROW, cc, 136, lane);
 }
 
 // helper warps: publish the tile q-column by q-column (which = 0) and q-row by q-row (which = 1) (step a6
