@@ -282,6 +282,12 @@ def main():
         e2e_s = float(t.item())
     assert sc_e2e == score
 
+    # ---- N > 1: the workload that shards: cfg4, sequences dealt longest-first round-robin to the ranks,
+    # each rank folds its shard through rna4r_fold_batch_host, no data-path collective (scores gathered host-side)
+    sharded = None
+    if world > 1:
+        sharded = sharded_batch(pkg, torch, dist, r, rank, world, barrier, args.steps)
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -306,14 +312,32 @@ def main():
                 "peak_gbs": peaks["hbm_gbs"], "frac": alg_bytes / (fill_avg_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                 "note": "not the binding roofline: the fold reads n bytes and writes 4"},
     }
-    # optional ncu-measured DRAM traffic of the same kernel (profiles/), per launch
+    # DRAM traffic of the same kernel, per launch: an ncu counter cannot be read inside an un-profiled run, so this
+    # is the committed value of the latest `ncu --set full` capture (profiles/traffic.json names the capture)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
+    if os.path.exists(tpath) and CFG == "cfg3" and args.engine == "tiled":
         try:
             with open(tpath) as f:
-                roofline["traffic"] = json.load(f).get("cfg3_fill_kernel_dram_bytes")
+                tj = json.load(f)
+            roofline["traffic"] = tj.get("cfg3_fill_kernel_dram_bytes")
+            roofline["traffic_source"] = "static: " + str(tj.get("source")) + " (not measured by this run)"
         except Exception:
             pass
+    # measured ceiling of the lookup sequence itself (rna4r_microbench_lookups): what the SM sustains for the bare
+    # 4-instruction lookup, and for the bulk product's inner loop, conflict-free on every SM
+    if not args.profile and args.engine == "tiled":
+        try:
+            ceil = {}
+            for name, variant in (("pure_4_instr_lookup", 0), ("bulk_product_inner_loop", 1)):
+                best = 0.0
+                for _ in range(3):
+                    ms, nl = r.microbench_lookups(variant, 4000 if variant == 0 else 500)
+                    best = max(best, nl / (ms * 1e-3))
+                ceil[name] = {"glookups_per_s": best / 1e9, "frac_of_formula_peak": best / peak_lookups}
+            roofline["measured_ceiling"] = ceil
+            roofline["frac_of_measured_ceiling"] = ach_lookups / (ceil["pure_4_instr_lookup"]["glookups_per_s"] * 1e9)
+        except Exception as e:       # profiling aid only
+            roofline["measured_ceiling"] = {"error": str(e)}
 
     out = {
         "metric": "cell_k_updates_per_s", "value": value, "unit": "cell-k-updates/s",
@@ -333,6 +357,8 @@ def main():
         "paper_context": {"tesla_c2070_s": 2.50, "geforce_gtx550ti_s": 4.97, "cite": "PAPER.md:345"},
     }
 
+    if sharded is not None:
+        out["batch_sharded"] = sharded
     if args.profile:
         args.no_also = args.no_cpu = True
     if not args.no_also and world == 1:
@@ -347,6 +373,35 @@ def main():
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def sharded_batch(pkg, torch, dist, r, rank, world, barrier, steps):
+    """cfg4 sharded by sequence over the ranks (paper_1307_7820_b200/shard.py); value = sum W / max-rank time."""
+    from paper_1307_7820_b200 import shard
+    seqs, lens = workloads.gc_rich_batch()
+    idx = shard.shard_indices(lens, world, rank)
+    mine = [seqs[i] for i in idx]
+    flat, _, lens32 = workloads.pack_batch(mine)
+    pinned = torch.from_numpy(flat).pin_memory()
+    out_p = torch.zeros(len(lens32), dtype=torch.int32).pin_memory()
+    ws = torch.empty(r.workspace_bytes_host(lens32), dtype=torch.uint8, device="cuda")
+    for _ in range(3):
+        r.fold_batch_host(pinned, lens32, workspace=ws, scores_host=out_p)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        sc = r.fold_batch_host(pinned, lens32, workspace=ws, scores_host=out_p)
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / steps
+    t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tot = torch.tensor([float(sc.sum())], device="cuda", dtype=torch.float64)
+    dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    wtot = int(sum(nussinov_updates(int(x)) for x in lens))
+    return {"workload": "cfg4: 1024 sequences, lengths U[300,700], sharded by sequence (longest first, round robin), "
+                        "rna4r_fold_batch_host per rank, no collective on the data path",
+            "value": wtot / float(t.item()), "unit": "cell-k-updates/s", "seconds_per_batch_max_rank": float(t.item()),
+            "sum_scores": int(tot.item()), "scaling": "strong"}
 
 
 def also_workloads(pkg, torch, r8, flush):
@@ -407,6 +462,20 @@ def also_workloads(pkg, torch, r8, flush):
     res["cfg4_batch1024_q8"] = {"ms": ms, "cell_k_updates_per_s": wtot / (ms * 1e-3), "fill_kernel_ms": r8.last_fill_kernel_ms(),
                                "lookups": ltot, "sum_scores": int(sc.sum().item())}
     del wsb
+    # the same batch end to end: pinned host buffers through rna4r_fold_batch_host, copies inside the timed region
+    pinned = torch.from_numpy(flat).pin_memory()
+    out_p = torch.zeros(len(lens32), dtype=torch.int32).pin_memory()
+    wsh = torch.empty(r8.workspace_bytes_host(lens32), dtype=torch.uint8, device="cuda")
+    for _ in range(3):
+        r8.fold_batch_host(pinned, lens32, workspace=wsh, scores_host=out_p)
+    t0 = time.perf_counter()
+    for _ in range(10):
+        r8.fold_batch_host(pinned, lens32, workspace=wsh, scores_host=out_p)
+    e2e_s = (time.perf_counter() - t0) / 10
+    res["cfg4_batch1024_q8"]["e2e"] = {"value": wtot / e2e_s, "unit": "cell-k-updates/s", "seconds_per_batch": e2e_s,
+                                        "h2d_bytes_per_step": int(flat.size + 4 * len(lens32)), "d2h_bytes_per_step": int(4 * len(lens32)),
+                                        "sum_scores": int(out_p.sum().item())}
+    del wsh
     # cfg5
     s = workloads.single_config("cfg5")
     d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()

@@ -32,6 +32,10 @@
  *   - Input alphabet: bytes A C G U, lower case accepted, T == U.  Any other byte makes that
  *     sequence's score -1 (and, for rna4r_fold, leaves table_out unspecified); other sequences
  *     of a batch are unaffected.  n = 0 and n = 1 are valid and score 0.
+ *   - Errors that only the device can see (a byte that is not a base; device offsets that disagree
+ *     with lens_host) never fail the call: the sequence's score is -1 and, when the caller passes a
+ *     status array (rna4r_fold_batch_status), its status word holds the RNA4R_STATUS_* bits.  A
+ *     single fold (rna4r_fold) reports through the score alone: -1 means RNA4R_STATUS_BAD_BASE.
  */
 #ifndef RNA4R_H
 #define RNA4R_H
@@ -54,6 +58,17 @@ extern "C" {
 #define RNA4R_ERR_DEVICE     -7   /* no CUDA device, or the device is not compute capability 10.x */
 #define RNA4R_ERR_DTYPE      -8   /* table_dtype not one of RNA4R_TABLE_*                      */
 #define RNA4R_ERR_ENGINE     -9   /* engine id unknown, or the engine does not support this q  */
+
+/* ---- per-sequence status bits (device-detected; see rna4r_fold_batch_status) ---- */
+#define RNA4R_STATUS_OK           0
+#define RNA4R_STATUS_BAD_BASE     1   /* the sequence holds a byte outside A C G U T (either case)          */
+#define RNA4R_STATUS_BAD_OFFSETS  2   /* offsets_dev[t+1]-offsets_dev[t] != lens_host[t]: sequence not read */
+
+/* ---- rna4r_workspace_bytes flags ---- */
+#define RNA4R_WS_DEVICE        0      /* device-buffer calls (rna4r_fold, rna4r_fold_batch)                 */
+#define RNA4R_WS_HOST_STAGING  1      /* + staging for the *_host variants (bases, offsets, scores)        */
+#define RNA4R_WS_HOST_TABLE16  2      /* + staging for rna4r_fold_host's int16 table (count == 1 only)     */
+#define RNA4R_WS_HOST_TABLE32  4      /* + staging for rna4r_fold_host's int32 table (count == 1 only)     */
 
 /* ---- table_out element types ---- */
 #define RNA4R_TABLE_NONE   0
@@ -105,12 +120,24 @@ int rna4r_engine(const rna4r_ctx *ctx);   /* the engine fold calls will use (res
 
 /*
  * Workspace size in bytes for `count` sequences each of length <= n_max with the context's current
- * engine (an upper bound; 0 on error).  rna4r_workspace_bytes_batch gives the exact size for given
- * lengths (lens_host: host int32[count]).  The workspace needs 256-byte alignment and holds only
- * scratch: its contents are undefined before and after a call.
+ * engine (an upper bound; 0 on error).  flags: RNA4R_WS_DEVICE, or RNA4R_WS_HOST_* bits OR-ed to add
+ * the staging area of the *_host variants.  rna4r_workspace_bytes_batch gives the exact device-side
+ * size for given lengths (lens_host: host int32[count]); rna4r_workspace_bytes_host (below) the exact
+ * size for the *_host variants.  The workspace needs 256-byte alignment and holds only scratch: its
+ * contents are undefined before and after a call.
  */
-size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count);
+size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count, int flags);
 size_t rna4r_workspace_bytes_batch(const rna4r_ctx *ctx, const int32_t *lens_host, int count);
+
+/*
+ * Caps the number of CTAs per SM the persistent fill kernel of the TILED engine is launched with
+ * (a tuning / test knob: a smaller grid changes the interleaving of the wavefront tasks, never the
+ * result).  0 = no cap (the default: as many as fit).  Errors: CONTEXT, BAD_N (negative).
+ */
+int rna4r_set_max_blocks_per_sm(rna4r_ctx *ctx, int blocks_per_sm);
+/* The same for the whole grid (0 = no cap).  Any grid >= 1 CTA completes: a claimed task only waits on tasks
+ * claimed earlier.  Errors: CONTEXT, BAD_N. */
+int rna4r_set_max_blocks(rna4r_ctx *ctx, int blocks);
 
 /*
  * rna4r_fold -- one fold (problem statement PAPER.md:45-54; wavefront PAPER.md:223-269).
@@ -133,14 +160,23 @@ int rna4r_fold(rna4r_ctx *ctx, const uint8_t *seq_dev, int n,
  *   seqs_dev       device uint8[offsets[count]]: concatenated bases.
  *   offsets_dev    device int64[count+1]: start offsets, offsets[0] = 0, non-decreasing.
  *   lens_host      HOST int32[count]: lens_host[t] = offsets[t+1]-offsets[t]; host memory so the
- *                  library can size and validate the work without a device synchronisation.
+ *                  library can size and validate the work without a device synchronisation.  It is
+ *                  consumed (copied) before the call returns.  The geometry of the work always
+ *                  follows lens_host; a sequence whose device offsets disagree is not read and
+ *                  scores -1 (RNA4R_STATUS_BAD_OFFSETS).
  *   scores_out_dev device int32[count]: D(1,n_t) per sequence (-1 for an invalid sequence).
+ *   status_out_dev (rna4r_fold_batch_status only) device int32[count] or NULL: RNA4R_STATUS_* bits
+ *                  per sequence, 0 = folded.
  *   workspace_dev  device scratch of >= rna4r_workspace_bytes_batch(ctx, lens_host, count).
  * Errors: CONTEXT, NULL, BAD_N, WORKSPACE, CUDA.
  */
 int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *offsets_dev,
                      const int32_t *lens_host, int count, int32_t *scores_out_dev,
                      void *workspace_dev, size_t workspace_bytes, void *stream);
+int rna4r_fold_batch_status(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *offsets_dev,
+                            const int32_t *lens_host, int count, int32_t *scores_out_dev,
+                            int32_t *status_out_dev,
+                            void *workspace_dev, size_t workspace_bytes, void *stream);
 
 /*
  * rna4r_traceback -- one optimal structure (a maximum set of non-crossing complementary pairs) from a
@@ -164,9 +200,11 @@ int rna4r_traceback(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, const void *t
 /*
  * Host-buffer variants (the end-to-end path): the sequence(s) are copied host->device into the
  * workspace, folded, the score(s) (and table) copied device->host, and `stream` is synchronised
- * before returning.  Host buffers should be pinned for full copy bandwidth but need not be.
- * Workspace: rna4r_workspace_bytes_host(ctx, total_bases, count, table_elems_bytes) extra bytes on
- * top of the device-side requirement are included by the *_host size queries below.
+ * before returning (once, at the end; no host allocation).  Host buffers should be pinned for full
+ * copy bandwidth but need not be.
+ * Workspace: rna4r_workspace_bytes_host(ctx, lens_host, count, table_dtype) = the device-side
+ * requirement for these lengths plus the staging area (bases, offsets, scores, and -- count == 1,
+ * table_dtype != RNA4R_TABLE_NONE -- the n*n table); 0 on error.
  *   table_out_host (rna4r_fold_host only): host n*n elements or NULL.
  */
 size_t rna4r_workspace_bytes_host(const rna4r_ctx *ctx, const int32_t *lens_host, int count, int table_dtype);
@@ -202,6 +240,22 @@ int rna4r_last_fill_kernel_ms(rna4r_ctx *ctx, float *ms_host);
  */
 int rna4r_set_trace(rna4r_ctx *ctx, int max_tiles);
 int rna4r_trace_to_host(rna4r_ctx *ctx, uint64_t *dst_host, int tiles);
+
+/*
+ * Measured ceiling of the lookup sequence (a profiling aid for the roofline denominator).
+ * Runs, from every SM and free of bank conflicts, the instruction sequence of one table lookup of eq. (3)
+ * as the fill kernel issues it, and times it with CUDA events on `stream` (synchronises):
+ *   variant 0 (context q = 8):  add, address, 1-byte shared-memory gather, add-max; operands in registers;
+ *   variant 1 (context q = 8):  the bulk product's inner loop (operand words loaded from shared memory);
+ *   variant 2 (context q = 10): the nibble-table sequence; operands in registers.
+ *   iters           loop trips per thread, 1..16000 (16 lookups per trip; variant 1: 128 per trip).
+ *   blocks_per_sm   CTAs of 256 threads per SM (0 = as many as fit).
+ *   workspace_dev   device scratch, >= 256 bytes.
+ *   ms_host, lookups_host   HOST outputs: elapsed milliseconds and the number of lookups executed.
+ * Errors: CONTEXT, NULL, BAD_N, ENGINE (variant does not match the context's q), CUDA.
+ */
+int rna4r_microbench_lookups(rna4r_ctx *ctx, int variant, int iters, int blocks_per_sm, void *workspace_dev,
+                             void *stream, float *ms_host, double *lookups_host);
 
 /* cudaError_t of the most recent failing CUDA call on this context (0 if none). */
 int rna4r_last_cuda_error(const rna4r_ctx *ctx);

@@ -49,7 +49,12 @@ def load():
     L.rna4r_table_to_host.argtypes = [vp, vp, ctypes.c_int]
     L.rna4r_set_engine.argtypes = [vp, ctypes.c_int]
     L.rna4r_engine.argtypes = [vp]
-    L.rna4r_workspace_bytes.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    L.rna4r_workspace_bytes.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+    L.rna4r_set_max_blocks_per_sm.argtypes = [vp, ctypes.c_int]
+    L.rna4r_set_max_blocks.argtypes = [vp, ctypes.c_int]
+    L.rna4r_microbench_lookups.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp,
+                                           ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
+    L.rna4r_fold_batch_status.argtypes = [vp, u8p, i64p, i32p, ctypes.c_int, i32p, i32p, vp, ctypes.c_size_t, vp]
     L.rna4r_workspace_bytes.restype = ctypes.c_size_t
     L.rna4r_workspace_bytes_batch.argtypes = [vp, i32p, ctypes.c_int]
     L.rna4r_workspace_bytes_batch.restype = ctypes.c_size_t
@@ -142,6 +147,17 @@ class Rna4r:
         _check(self.lib.rna4r_last_fill_kernel_ms(self.h, ctypes.byref(ms)), "rna4r_last_fill_kernel_ms")
         return float(ms.value)
 
+    def set_max_blocks(self, blocks: int):
+        _check(self.lib.rna4r_set_max_blocks(self.h, int(blocks)), "rna4r_set_max_blocks")
+
+    def microbench_lookups(self, variant: int, iters: int = 4000, blocks_per_sm: int = 0, stream=None):
+        """rna4r_microbench_lookups: (milliseconds, lookups executed) of the bare lookup sequence on every SM."""
+        ms, n = ctypes.c_float(0), ctypes.c_double(0)
+        ws = self.workspace(256)
+        _check(self.lib.rna4r_microbench_lookups(self.h, variant, iters, blocks_per_sm, ws.data_ptr(), _stream_ptr(stream),
+                                                 ctypes.byref(ms), ctypes.byref(n)), "rna4r_microbench_lookups")
+        return float(ms.value), float(n.value)
+
     def set_trace(self, max_tiles: int):
         _check(self.lib.rna4r_set_trace(self.h, int(max_tiles)), "rna4r_set_trace")
 
@@ -162,8 +178,11 @@ class Rna4r:
             self._ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=f"cuda:{self.device}")
         return self._ws
 
-    def workspace_bytes(self, n_max: int, count: int = 1) -> int:
-        return self.lib.rna4r_workspace_bytes(self.h, n_max, count)
+    def workspace_bytes(self, n_max: int, count: int = 1, flags: int = 0) -> int:
+        return self.lib.rna4r_workspace_bytes(self.h, n_max, count, flags)
+
+    def set_max_blocks_per_sm(self, blocks_per_sm: int):
+        _check(self.lib.rna4r_set_max_blocks_per_sm(self.h, int(blocks_per_sm)), "rna4r_set_max_blocks_per_sm")
 
     def workspace_bytes_batch(self, lens: np.ndarray) -> int:
         lens = np.ascontiguousarray(lens, dtype=np.int32)
@@ -192,8 +211,10 @@ class Rna4r:
                                    workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)), "rna4r_fold")
         return score_out, table_out
 
-    def fold_batch(self, seqs_dev, offsets_dev, lens_host: np.ndarray, scores_out=None, workspace=None, stream=None):
-        """rna4r_fold_batch.  Enqueues only; returns the int32[count] score tensor."""
+    def fold_batch(self, seqs_dev, offsets_dev, lens_host: np.ndarray, scores_out=None, workspace=None, stream=None,
+                   status_out=None):
+        """rna4r_fold_batch (rna4r_fold_batch_status when status_out, an int32[count] CUDA tensor, is given).
+        Enqueues only; returns the int32[count] score tensor."""
         import torch
         lens_host = np.ascontiguousarray(lens_host, dtype=np.int32)
         count = len(lens_host)
@@ -201,9 +222,14 @@ class Rna4r:
             scores_out = torch.empty(max(count, 1), dtype=torch.int32, device=f"cuda:{self.device}")
         if workspace is None:
             workspace = self.workspace(self.workspace_bytes_batch(lens_host))
-        _check(self.lib.rna4r_fold_batch(self.h, seqs_dev.data_ptr(), offsets_dev.data_ptr(), lens_host.ctypes.data, count,
-                                         scores_out.data_ptr(), workspace.data_ptr(), workspace.numel(),
-                                         _stream_ptr(stream)), "rna4r_fold_batch")
+        if status_out is not None:
+            _check(self.lib.rna4r_fold_batch_status(self.h, seqs_dev.data_ptr(), offsets_dev.data_ptr(), lens_host.ctypes.data,
+                                                    count, scores_out.data_ptr(), status_out.data_ptr(), workspace.data_ptr(),
+                                                    workspace.numel(), _stream_ptr(stream)), "rna4r_fold_batch_status")
+        else:
+            _check(self.lib.rna4r_fold_batch(self.h, seqs_dev.data_ptr(), offsets_dev.data_ptr(), lens_host.ctypes.data, count,
+                                             scores_out.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                             _stream_ptr(stream)), "rna4r_fold_batch")
         return scores_out[:count]
 
     # -- traceback --------------------------------------------------------------------------------

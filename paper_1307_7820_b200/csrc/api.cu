@@ -4,6 +4,7 @@
 #include "diag_engine.cuh"
 #include "tiled_engine.cuh"
 #include "traceback.cuh"
+#include "microbench.cuh"
 
 #include <new>
 
@@ -95,14 +96,14 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return RNA4R_ERR_DEVICE;
-    if (prop.major != 10) return RNA4R_ERR_DEVICE;   // sm_100a code only; no fallback path exists
+    if (prop.major != 10 || prop.minor != 0) return RNA4R_ERR_DEVICE;   // the library holds sm_100a code only; no fallback path exists
     rna4r_ctx *ctx = new (std::nothrow) rna4r_ctx();
     if (!ctx) return RNA4R_ERR_CUDA;
     ctx->magic = RNA4R_MAGIC; ctx->q = q; ctx->device = device;
     ctx->engine = (q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
     ctx->sm_count = prop.multiProcessorCount;
     ctx->R = ctx->Rc = ctx->Rc4 = nullptr;
-    ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0;
+    ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0; ctx->max_blocks_per_sm = 0; ctx->max_blocks = 0;
     ctx->timing = 0; ctx->timing_valid = 0; ctx->ev0 = ctx->ev1 = nullptr;
     ctx->trace = nullptr; ctx->trace_tiles = 0;
     cudaStream_t st = (cudaStream_t)stream;
@@ -115,10 +116,11 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     if ((e = cudaMalloc(&ctx->Rc4, M * M / 2 < 16 ? 16 : M * M / 2)) != cudaSuccess) return fail(e);
     {
         const size_t total = N * N;
-        int blocks = (int)((total + 255) / 256); if (blocks > 148 * 16) blocks = 148 * 16;
+        const int cap = ctx->sm_count * 16;
+        int blocks = (int)((total + 255) / 256); if (blocks > cap) blocks = cap;
         rna4r_build_rtable_kernel<<<blocks, 256, 0, st>>>(q, ctx->R);
         const size_t tc = M * M;
-        blocks = (int)((tc + 255) / 256); if (blocks > 148 * 16) blocks = 148 * 16;
+        blocks = (int)((tc + 255) / 256); if (blocks > cap) blocks = cap;
         rna4r_build_compact_kernel<<<blocks, 256, 0, st>>>(q, ctx->R, ctx->Rc);
         rna4r_pack_nibbles_kernel<<<blocks, 256, 0, st>>>(tc, ctx->Rc, ctx->Rc4);
         if ((e = cudaGetLastError()) != cudaSuccess) return fail(e);
@@ -219,15 +221,39 @@ int rna4r_set_engine(rna4r_ctx *ctx, int engine)
     return RNA4R_OK;
 }
 
-size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count)
+int rna4r_set_max_blocks_per_sm(rna4r_ctx *ctx, int blocks_per_sm)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (blocks_per_sm < 0) return RNA4R_ERR_BAD_N;
+    ctx->max_blocks_per_sm = blocks_per_sm;
+    return RNA4R_OK;
+}
+
+int rna4r_set_max_blocks(rna4r_ctx *ctx, int blocks)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (blocks < 0) return RNA4R_ERR_BAD_N;
+    ctx->max_blocks = blocks;
+    return RNA4R_OK;
+}
+
+static size_t host_staging_bytes(size_t total_bases, int count, size_t table_bytes);
+
+size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count, int flags)
 {
     if (!ctx_ok(ctx) || n_max < 0 || count < 0 || n_max > 65534) return 0;
-    if (count == 0) return 256;
-    if (ctx->engine == RNA4R_ENGINE_TILED) {
+    if (flags & ~(RNA4R_WS_HOST_STAGING | RNA4R_WS_HOST_TABLE16 | RNA4R_WS_HOST_TABLE32)) return 0;
+    size_t core = 256;
+    if (count > 0) {
         // every sequence at n_max: per-sequence cost is monotone in n
-        return (size_t)count * (tiled_ws(ctx, nullptr, 1, n_max)) ;
+        if (ctx->engine == RNA4R_ENGINE_TILED) core = (size_t)count * tiled_ws(ctx, nullptr, 1, n_max);
+        else core = (size_t)count * diag_ws_layout(nullptr, n_max).bytes;
     }
-    return (size_t)count * diag_ws_layout(nullptr, n_max).bytes;
+    if (!(flags & (RNA4R_WS_HOST_STAGING | RNA4R_WS_HOST_TABLE16 | RNA4R_WS_HOST_TABLE32))) return core;
+    size_t table_bytes = 0;
+    if (count == 1 && (flags & RNA4R_WS_HOST_TABLE32)) table_bytes = (size_t)n_max * n_max * 4;
+    else if (count == 1 && (flags & RNA4R_WS_HOST_TABLE16)) table_bytes = (size_t)n_max * n_max * 2;
+    return align_up(core, 256) + host_staging_bytes((size_t)count * n_max, count, table_bytes);
 }
 
 size_t rna4r_workspace_bytes_batch(const rna4r_ctx *ctx, const int32_t *lens_host, int count)
@@ -251,19 +277,27 @@ int rna4r_fold(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_out
     cudaStream_t st = (cudaStream_t)stream;
     RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
     if (ctx->engine == RNA4R_ENGINE_DIAG)
-        return diag_fold_enqueue(ctx, seq_dev, n, score_out_dev, table_out_dev, table_dtype, workspace_dev, st);
+        return diag_fold_enqueue(ctx, seq_dev, nullptr, n, score_out_dev, nullptr, table_out_dev, table_dtype, workspace_dev, st);
     if (table_out_dev && n > 0) {
         const size_t es = table_dtype == RNA4R_TABLE_INT16 ? 2 : 4;
         RNA4R_CUDA(ctx, cudaMemsetAsync(table_out_dev, 0, (size_t)n * n * es, st));   // zeros below the diagonal
     }
     return dispatch_q(ctx->q, [&](auto Q) {
-        return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seq_dev, nullptr, nullptr, 1, n, score_out_dev,
+        return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seq_dev, nullptr, nullptr, 1, n, score_out_dev, nullptr,
                                                     table_out_dev, table_dtype, workspace_dev, st);
     });
 }
 
 int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *offsets_dev, const int32_t *lens_host,
                      int count, int32_t *scores_out_dev, void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    return rna4r_fold_batch_status(ctx, seqs_dev, offsets_dev, lens_host, count, scores_out_dev, nullptr, workspace_dev,
+                                   workspace_bytes, stream);
+}
+
+int rna4r_fold_batch_status(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *offsets_dev, const int32_t *lens_host,
+                            int count, int32_t *scores_out_dev, int32_t *status_out_dev, void *workspace_dev,
+                            size_t workspace_bytes, void *stream)
 {
     if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
     if (count < 0) return RNA4R_ERR_BAD_N;
@@ -280,14 +314,14 @@ int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *off
     cudaStream_t st = (cudaStream_t)stream;
     RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
     if (ctx->engine == RNA4R_ENGINE_DIAG) {
-        size_t off = 0, ws_off = 0;
+        size_t ws_off = 0;            // sequence t starts at offsets_dev[t] (read on the device)
         int launches = 0;
         for (int t = 0; t < count; ++t) {
-            int rc = diag_fold_enqueue(ctx, seqs_dev + off, lens_host[t], scores_out_dev + t, nullptr, RNA4R_TABLE_NONE,
+            int rc = diag_fold_enqueue(ctx, seqs_dev, offsets_dev + t, lens_host[t], scores_out_dev + t,
+                                       status_out_dev ? status_out_dev + t : nullptr, nullptr, RNA4R_TABLE_NONE,
                                        (char *)workspace_dev + ws_off, st);
             if (rc != RNA4R_OK) return rc;
             launches += ctx->last_launches;
-            off += (size_t)lens_host[t];
             ws_off += diag_ws_layout(nullptr, lens_host[t]).bytes;
         }
         ctx->last_launches = launches;
@@ -295,8 +329,24 @@ int rna4r_fold_batch(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64_t *off
     }
     return dispatch_q(ctx->q, [&](auto Q) {
         return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
-                                                    nullptr, RNA4R_TABLE_NONE, workspace_dev, st);
+                                                    status_out_dev, nullptr, RNA4R_TABLE_NONE, workspace_dev, st);
     });
+}
+
+// ---- measured ceiling of the lookup sequence (profiling aid; microbench.cuh) ------------------------------------
+int rna4r_microbench_lookups(rna4r_ctx *ctx, int variant, int iters, int blocks_per_sm, void *workspace_dev, void *stream,
+                             float *ms_host, double *lookups_host)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (!workspace_dev || !ms_host || !lookups_host) return RNA4R_ERR_NULL;
+    if (iters < 1 || iters > 16000) return RNA4R_ERR_BAD_N;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    uint32_t *sink = (uint32_t *)workspace_dev;
+    if (variant == 0 && ctx->q == 8) return microbench::run<8, 0>(ctx, iters, blocks_per_sm, sink, st, ms_host, lookups_host);
+    if (variant == 1 && ctx->q == 8) return microbench::run<8, 1>(ctx, iters, blocks_per_sm, sink, st, ms_host, lookups_host);
+    if (variant == 2 && ctx->q == 10) return microbench::run<10, 0>(ctx, iters, blocks_per_sm, sink, st, ms_host, lookups_host);
+    return RNA4R_ERR_ENGINE;
 }
 
 // ---- traceback: one optimal structure from a finished table ------------------------
@@ -335,6 +385,28 @@ int rna4r_traceback(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, const void *t
 }
 
 // ---- host-buffer variants: staging area at the END of the workspace --------------------------------
+// offsets[0..count] = exclusive prefix sum of lens[0..count) (one block; count is at most a few 10^5)
+__global__ void rna4r_offsets_from_lens_kernel(const int32_t *__restrict__ lens, int count, int64_t *__restrict__ offsets)
+{
+    __shared__ long long part[1024];
+    const int tid = threadIdx.x, nth = blockDim.x;
+    const int per = (count + nth - 1) / nth;
+    const int lo = min(tid * per, count), hi = min(lo + per, count);
+    long long sum = 0;
+    for (int t = lo; t < hi; ++t) sum += lens[t];
+    part[tid] = sum;
+    __syncthreads();
+    for (int d = 1; d < nth; d <<= 1) {          // inclusive scan of the per-thread sums
+        const long long v = (tid >= d) ? part[tid - d] : 0;
+        __syncthreads();
+        part[tid] += v;
+        __syncthreads();
+    }
+    long long run = part[tid] - sum;
+    for (int t = lo; t < hi; ++t) { offsets[t] = run; run += lens[t]; }
+    if (tid == nth - 1) offsets[count] = part[nth - 1];
+}
+
 static size_t host_staging_bytes(size_t total_bases, int count, size_t table_bytes)
 {
     return align_up(total_bases + 16, 256) + align_up((size_t)(count + 1) * 8, 256) + align_up((size_t)count * 4 + 16, 256) + align_up(table_bytes, 256);
@@ -405,19 +477,14 @@ int rna4r_fold_batch_host(rna4r_ctx *ctx, const uint8_t *seqs_host, const int32_
     uint8_t *seqs_dev = (uint8_t *)stg; stg += align_up(total_bases + 16, 256);
     int64_t *offs_dev = (int64_t *)stg; stg += align_up((size_t)(count + 1) * 8, 256);
     int32_t *scores_dev = (int32_t *)stg;
-    // offsets are derived from lens on the host (count+1 int64) and copied with the bases
-    int64_t *offs_host = new (std::nothrow) int64_t[(size_t)count + 1];
-    if (!offs_host) return RNA4R_ERR_CUDA;
-    offs_host[0] = 0;
-    for (int t = 0; t < count; ++t) offs_host[t + 1] = offs_host[t] + lens_host[t];
-    cudaError_t e = cudaMemcpyAsync(offs_dev, offs_host, (size_t)(count + 1) * 8, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess && total_bases) e = cudaMemcpyAsync(seqs_dev, seqs_host, total_bases, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // offs_host is pageable: make sure the copy has consumed it
-    delete[] offs_host;
-    if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return RNA4R_ERR_CUDA; }
+    // The offsets are an exclusive scan of the lengths, done on the device: the lengths travel in the (still unused)
+    // score slots, so the call needs no host scratch and synchronises once, at the end.
+    RNA4R_CUDA(ctx, cudaMemcpyAsync(scores_dev, lens_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
+    if (total_bases) RNA4R_CUDA(ctx, cudaMemcpyAsync(seqs_dev, seqs_host, total_bases, cudaMemcpyHostToDevice, st));
+    rna4r_offsets_from_lens_kernel<<<1, 1024, 0, st>>>(scores_dev, count, offs_dev);
     int rc = rna4r_fold_batch(ctx, seqs_dev, offs_dev, lens_host, count, scores_dev, workspace_dev, core, st);
     if (rc != RNA4R_OK) return rc;
-    const int launches = ctx->last_launches;
+    const int launches = ctx->last_launches + 1;
     RNA4R_CUDA(ctx, cudaMemcpyAsync(scores_out_host, scores_dev, (size_t)count * 4, cudaMemcpyDeviceToHost, st));
     RNA4R_CUDA(ctx, cudaStreamSynchronize(st));
     ctx->last_launches = launches;

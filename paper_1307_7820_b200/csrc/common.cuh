@@ -17,6 +17,8 @@ struct rna4r_ctx {
     int last_launches;
     int last_cuda_error;
     int tiled_blocks_per_sm; // occupancy of the tiled fill kernel for this q (0 = not queried yet)
+    int max_blocks_per_sm;   // rna4r_set_max_blocks_per_sm: cap on resident CTAs per SM of the fill kernel (0 = none)
+    int max_blocks;          // rna4r_set_max_blocks: cap on the whole grid of the fill kernel (0 = none)
     int timing;              // record events around the dominant kernel
     int timing_valid;
     cudaEvent_t ev0, ev1;

@@ -41,12 +41,20 @@ static inline DiagWs diag_ws_layout(void *base, int n)
     return w;
 }
 
-__global__ void diag_encode_kernel(const uint8_t *__restrict__ seq, int n, int8_t *__restrict__ codes, int *invalid)
+// `offset` (device, may be NULL): offset[0] = start of the sequence in seq, offset[1] = its end (a batch member);
+// a length that disagrees with n (from lens_host) is reported instead of read (RNA4R_STATUS_BAD_OFFSETS).
+__global__ void diag_encode_kernel(const uint8_t *__restrict__ seq, const int64_t *__restrict__ offset, int n,
+                                   int8_t *__restrict__ codes, int *invalid)
 {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n) return;
-    int c = rna4r_base_code(seq[t]);
-    if (c == 4) atomicOr(invalid, 1);
+    int64_t start = 0;
+    if (offset) {
+        start = offset[0];
+        if (offset[1] - start != (int64_t)n) { if (t == 0) atomicOr(invalid, RNA4R_STATUS_BAD_OFFSETS); codes[t + 1] = 4; return; }
+    }
+    int c = rna4r_base_code(seq[start + t]);
+    if (c == 4) atomicOr(invalid, RNA4R_STATUS_BAD_BASE);
     codes[t + 1] = (int8_t)c;
 }
 
@@ -97,10 +105,17 @@ __global__ void diag_fill_kernel(int n, int q, int d, const int8_t *__restrict__
 }
 
 // D(1,n) -> score (or -1), and the optional row-major table.
-__global__ void diag_score_kernel(int n, const int16_t *__restrict__ Dd, const int *invalid, int32_t *score)
+__global__ void diag_score_kernel(int n, const int16_t *__restrict__ Dd, const int *invalid, int32_t *score, int32_t *status)
 {
     const size_t P = (size_t)n + 2;
     *score = *invalid ? -1 : (int32_t)Dd[(size_t)n * P + 1];   // diagonal n-1, row 1
+    if (status) *status = *invalid;
+}
+__global__ void diag_empty_kernel(const int64_t *__restrict__ offset, int32_t *score, int32_t *status)
+{
+    const int bad = (offset && offset[1] != offset[0]) ? RNA4R_STATUS_BAD_OFFSETS : 0;
+    *score = bad ? -1 : 0;
+    if (status) *status = bad;
 }
 
 template <typename OutT>
@@ -114,8 +129,8 @@ __global__ void diag_table_kernel(int n, const int16_t *__restrict__ Dd, OutT *_
     }
 }
 
-static int diag_fold_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_dev,
-                             void *table_out, int table_dtype, void *ws, cudaStream_t st)
+static int diag_fold_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, const int64_t *offset_dev, int n, int32_t *score_dev,
+                             int32_t *status_dev, void *table_out, int table_dtype, void *ws, cudaStream_t st)
 {
     DiagWs w = diag_ws_layout(ws, n);
     const size_t P = (size_t)n + 2;
@@ -123,7 +138,7 @@ static int diag_fold_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int3
     // zero: invalid flag, hrun, vrun, codes, and the two zero diagonals D(i,i-1) = D(i,i) = 0
     RNA4R_CUDA(ctx, cudaMemsetAsync(ws, 0, (size_t)((char *)w.Dd - (char *)ws) + 2 * P * sizeof(int16_t), st));
     if (n > 0) {
-        diag_encode_kernel<<<(n + 255) / 256, 256, 0, st>>>(seq_dev, n, w.codes, w.invalid);
+        diag_encode_kernel<<<(n + 255) / 256, 256, 0, st>>>(seq_dev, offset_dev, n, w.codes, w.invalid);
         ++launches;
     }
     const int q = ctx->q;
@@ -135,9 +150,10 @@ static int diag_fold_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int3
     }
     if (ctx->timing) { RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev1, st)); ctx->timing_valid = 1; }
     if (n == 0) {
-        RNA4R_CUDA(ctx, cudaMemsetAsync(score_dev, 0, sizeof(int32_t), st));
+        diag_empty_kernel<<<1, 1, 0, st>>>(offset_dev, score_dev, status_dev);
+        ++launches;
     } else {
-        diag_score_kernel<<<1, 1, 0, st>>>(n, w.Dd, w.invalid, score_dev);
+        diag_score_kernel<<<1, 1, 0, st>>>(n, w.Dd, w.invalid, score_dev, status_dev);
         ++launches;
     }
     if (table_out && n > 0) {

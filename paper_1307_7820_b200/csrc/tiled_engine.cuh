@@ -33,7 +33,6 @@
 // barrier per diagonal ("Synchronize with other processes").
 #pragma once
 #include "common.cuh"
-#include <cstdlib>
 
 namespace tiled {
 
@@ -136,6 +135,8 @@ constexpr int TASK_PROD = 1;
 struct Params {
     const uint8_t *seqs;
     const int64_t *offsets;   // device [count+1], or NULL for a single sequence of length n_single
+    const int32_t *lens_dev;  // device copy of lens_host [count] (batch only): the geometry always follows the host plan
+    int32_t *status;          // NULL, or device [count]: RNA4R_STATUS_* bits per sequence
     int n_single;
     int count;
     int max_nt;
@@ -160,6 +161,7 @@ struct Params {
     int table_dtype;
     unsigned long long *trace;   // NULL, or [tiles][8] phase stamps (ns) of the CLOSE tasks
     int trace_tiles;
+    int sm_count;                // SMs of the device (role rotation of co-resident CTAs)
 };
 
 __host__ __device__ inline int nstages(int dp, int delta)
@@ -182,11 +184,14 @@ __global__ void plan_seq_kernel(Params p)
     constexpr int T = Cfg<Q>::T;
     const int t = blockIdx.x;
     if (t >= p.count) return;
-    const int n = p.offsets ? (int)(p.offsets[t + 1] - p.offsets[t]) : p.n_single;
+    // The geometry follows lens_host (copied to lens_dev), as the host-side workspace plan does; a sequence whose
+    // device offsets disagree with it is folded as padding and reported (score -1, RNA4R_STATUS_BAD_OFFSETS).
+    const int n = p.offsets ? p.lens_dev[t] : p.n_single;
     const int nt = n / T + 1;
     if (threadIdx.x == 0) {
         SeqInfo si;
-        si.n = n; si.nt = nt; si.invalid = 0; si.pad[0] = si.pad[1] = si.pad[2] = 0;
+        si.n = n; si.nt = nt; si.pad[0] = si.pad[1] = si.pad[2] = 0;
+        si.invalid = (p.offsets && p.offsets[t + 1] - p.offsets[t] != (int64_t)n) ? RNA4R_STATUS_BAD_OFFSETS : 0;
         si.sbase = atomicAdd(&p.hdr->ntiles, nt * (nt + 1) / 2);
         si.cbase = atomicAdd(&p.hdr->ncodes, nt * T);
         p.seqinfo[t] = si;
@@ -245,17 +250,19 @@ template <int Q>
 __global__ void encode_kernel(Params p)
 {
     constexpr int T = Cfg<Q>::T;
-    const int t = blockIdx.y;
-    const SeqInfo si = p.seqinfo[t];
-    const int len = si.nt * T;
-    const uint8_t *src = p.seqs + (p.offsets ? p.offsets[t] : 0);
-    bool bad = false;
-    for (int x = blockIdx.x * blockDim.x + threadIdx.x; x < len; x += gridDim.x * blockDim.x) {
-        int c = 4;
-        if (x < si.n) { c = rna4r_base_code(src[x]); bad |= (c == 4); }
-        p.codes[si.cbase + x] = (int8_t)c;
+    for (int t = blockIdx.y; t < p.count; t += gridDim.y) {
+        const SeqInfo si = p.seqinfo[t];
+        const int len = si.nt * T;
+        const bool readable = !(si.invalid & RNA4R_STATUS_BAD_OFFSETS);      // never read through offsets that failed the check
+        const uint8_t *src = p.seqs + (p.offsets && readable ? p.offsets[t] : 0);
+        bool bad = false;
+        for (int x = blockIdx.x * blockDim.x + threadIdx.x; x < len; x += gridDim.x * blockDim.x) {
+            int c = 4;
+            if (x < si.n && readable) { c = rna4r_base_code(src[x]); bad |= (c == 4); }
+            p.codes[si.cbase + x] = (int8_t)c;
+        }
+        if (bad) atomicOr(&p.seqinfo[t].invalid, RNA4R_STATUS_BAD_BASE);
     }
-    if (bad) atomicOr(&p.seqinfo[t].invalid, 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -425,6 +432,13 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
 }
+// Data that another CTA wrote with generic-proxy stores (st.global.cg + release flag) and that this thread is about
+// to read through the async proxy (cp.async.bulk) needs a cross-proxy fence between the acquire of the flag and
+// the copy (PTX memory model, "async proxy"); without it the two accesses are formally unordered.
+__device__ __forceinline__ void fence_proxy_async_global()
+{
+    asm volatile("fence.proxy.async.global;" ::: "memory");
+}
 // TMA 1-D bulk copy global -> shared; completion is signalled on `bar` (complete_tx)
 __device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar)
 {
@@ -487,6 +501,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
                 const int s_ik = si.sbase + tri_index(nt, I, K), s_kj = si.sbase + tri_index(nt, K, J);
                 wait_flag_ge(p.done + s_ik, 1);
                 wait_flag_ge(p.done + s_kj, 1);
+                fence_proxy_async_global();       // generic-proxy writes of other CTAs (acquired above) -> async-proxy reads below
                 uint32_t *dst = sm.stg + (size_t)b * 2 * C::PANEL_WORDS;
                 mbar_expect_tx(full + b, 2 * PANEL_BYTES);
                 bulk_g2s(dst, rec_ptr<Q>(p, s_ik), PANEL_BYTES, full + b);                                   // PH of (I,K)
@@ -496,6 +511,7 @@ __device__ void run_prod(const Params &p, const Smem<Q> &sm, const SeqInfo &si, 
             if (s != S - 1) {
                 // earlier stages (they ran at earlier steps and own acc until their release): fetch their maxima
                 wait_flag_ge(p.accstage + sidx, S - 1 - s);
+                fence_proxy_async_global();
                 mbar_expect_tx(full + 3, (uint32_t)(C::T * C::T * 2));
                 bulk_g2s(sm.valraw, p.acc + (size_t)sidx * C::T * C::T, (uint32_t)(C::T * C::T * 2), full + 3);
             }
@@ -729,6 +745,7 @@ __device__ __forceinline__ int warp_wait_flag_ge(const int *flag, int v, int lan
     if (lane == 0) {
         while ((have = ld_acquire_gpu(flag)) < v) __nanosleep(32);     // every poll is an acquire: no second round trip once the flag is seen
     }
+    __syncwarp();                                                      // orders the other lanes' data loads after lane 0's acquire
     have = __shfl_sync(0xffffffffu, have, 0);
     return have < 8 ? have : 8;
 }
@@ -927,6 +944,7 @@ __device__ __forceinline__ void loader_loop(const int *flag, const uint32_t *src
         }
         loaded = hi;
         if (loaded < 8) {
+            __syncwarp();                                              // lane 0's acquire of `next` precedes everybody's next data loads
             have = min(__shfl_sync(0xffffffffu, next, 0), 8);
             if (have <= loaded) have = warp_wait_flag_ge(flag, loaded + 1, lane);
         }
@@ -1098,7 +1116,7 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
     // co-resident CTAs (block index apart by a multiple of the SM count) rotate the roles by two warps, so that
     // their closure warps land on different SM sub-partitions (warp id mod 4)
     constexpr int NWARP = C::NTHR / 32;
-    const int rot = 2 * ((blockIdx.x / 148) % 2);
+    const int rot = 2 * ((blockIdx.x / p.sm_count) % 2);
     const int warp = ((NWARP - 1) - (tid >> 5) + NWARP - rot) % NWARP, lane = tid & 31;
     CloseCtx cc;
     cc.dp = dp;
@@ -1216,8 +1234,10 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
                 }
             }
         }
-        if (I == 0 && J == n / T && tid == 0)
+        if (I == 0 && J == n / T && tid == 0) {
             p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
+            if (p.status) p.status[seq] = si.invalid;
+        }
         __syncthreads();               // orders every thread's stores before thread 0's releases (cumulative)
         if (tid == 0) {
             if (dp == 0) { st_release_gpu(cc.rowprogX, 8); st_release_gpu(cc.colprogX, 8); }
@@ -1313,7 +1333,7 @@ static inline HostPlan host_plan(int T, int delta, const int32_t *lens, int coun
 struct WsLayout {
     size_t zero_bytes;   // prefix that must be zeroed before every fold
     size_t off_hdr, off_stepC, off_stepP, off_curC, off_curP, off_done, off_accstage, off_rowprog, off_colprog;
-    size_t off_seqinfo, off_tasks, off_codes, off_recs, off_acc, total;
+    size_t off_seqinfo, off_lens, off_tasks, off_codes, off_recs, off_acc, total;
 };
 
 static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int count)
@@ -1331,6 +1351,7 @@ static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int co
     w.off_colprog = off; off += align_up(h.tiles * 4, 256);
     w.zero_bytes = off;
     w.off_seqinfo = off; off += align_up((size_t)count * sizeof(SeqInfo), 256);
+    w.off_lens = off; off += align_up((size_t)count * 4, 256);
     w.off_tasks = off; off += align_up(h.tasks * sizeof(int4), 256);
     w.off_codes = off; off += align_up(h.codes, 256);
     w.off_recs = off; off += align_up(h.tiles * (size_t)rec_bytes, 256);
@@ -1350,7 +1371,8 @@ static size_t workspace_bytes_q(int delta, const int32_t *lens, int count, int n
 
 template <int Q>
 static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64_t *offsets, const int32_t *lens_host,
-                     int count, int n_single, int32_t *scores, void *table_out, int table_dtype, void *ws, cudaStream_t st)
+                     int count, int n_single, int32_t *scores, int32_t *status, void *table_out, int table_dtype, void *ws,
+                     cudaStream_t st)
 {
     using C = Cfg<Q>;
     if (delta <= 0) delta = pick_delta(C::T, lens_host, count, n_single);
@@ -1359,6 +1381,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     char *base = (char *)ws;
     Params p;
     p.seqs = seqs; p.offsets = offsets; p.n_single = n_single; p.count = count; p.max_nt = h.max_nt; p.delta = delta;
+    p.lens_dev = (const int32_t *)(base + w.off_lens); p.status = status;
     p.hdr = (PlanHdr *)(base + w.off_hdr);
     p.stepC = (int *)(base + w.off_stepC); p.stepP = (int *)(base + w.off_stepP);
     p.curC = (int *)(base + w.off_curC); p.curP = (int *)(base + w.off_curP);
@@ -1372,6 +1395,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     p.tbl = C::NIBBLE ? ctx->Rc4 : ctx->Rc;
     p.scores = scores; p.table_out = table_out; p.table_dtype = table_dtype;
     p.trace = ctx->trace; p.trace_tiles = ctx->trace_tiles;
+    p.sm_count = ctx->sm_count;
 
     if (ctx->tiled_blocks_per_sm == 0)     // first launch of this context (one q, one device): opt in to the large shared window
         RNA4R_CUDA(ctx, cudaFuncSetAttribute(fill_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
@@ -1383,12 +1407,14 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     }
     int launches = 0;
     RNA4R_CUDA(ctx, cudaMemsetAsync(ws, 0, w.zero_bytes, st));
+    if (offsets)    // lens_host is consumed before this call returns (pageable memory is staged by the runtime)
+        RNA4R_CUDA(ctx, cudaMemcpyAsync(base + w.off_lens, lens_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
     plan_seq_kernel<Q><<<count, 64, 0, st>>>(p); ++launches;
     plan_scan_kernel<<<1, 32, 0, st>>>(p); ++launches;
     plan_fill_kernel<Q><<<count * h.max_nt, 64, 0, st>>>(p); ++launches;
     {
         const int maxlen = h.max_nt * C::T;
-        dim3 grid((maxlen + 255) / 256, count);
+        dim3 grid((maxlen + 255) / 256, count < 65535 ? count : 65535);
         encode_kernel<Q><<<grid, 256, 0, st>>>(p); ++launches;
     }
     size_t want = h.tasks;
@@ -1397,9 +1423,10 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     // neighbours on its SM (measured at n=6000: 1.98 ms with 2 CTAs/SM, 2.11 ms with 3; n=2000: 0.60 / 0.64); long folds and
     // batches are throughput-bound and take every CTA they can get (n=8000: 3.43 ms with 3, 3.48 with 2; n=16384: 18.8 / 21).
     if (count == 1 && h.max_nt <= 112 && per_sm > 2) per_sm = 2;
-    if (const char *e = getenv("RNA4R_BLOCKS_PER_SM")) { const int v = atoi(e); if (v >= 1 && v < per_sm) per_sm = v; }   // tuning knob
+    if (ctx->max_blocks_per_sm >= 1 && ctx->max_blocks_per_sm < per_sm) per_sm = ctx->max_blocks_per_sm;   // rna4r_set_max_blocks_per_sm
     int blocks = ctx->sm_count * per_sm;
     if ((size_t)blocks > want) blocks = (int)want;
+    if (ctx->max_blocks >= 1 && blocks > ctx->max_blocks) blocks = ctx->max_blocks;
     if (blocks < 1) blocks = 1;
     if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
     fill_kernel<Q><<<blocks, C::NTHR, C::SMEM_BYTES, st>>>(p); ++launches;

@@ -25,6 +25,20 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
         assert hasattr(lib, nm), nm
 
 
+def test_header_compiles_as_c_and_a_c_program_calls_the_abi(tmp_path):
+    """include/rna4r.h is a C header: a C99 program includes it, links librna4r.so and calls the GPU-free entry points."""
+    import subprocess
+    from paper_1307_7820_b200 import build
+    lib = build.build()
+    exe = str(tmp_path / "c_abi_check")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"),
+                           os.path.join(ROOT, "tests", "c_abi_check.c"), "-o", exe,
+                           "-L", os.path.dirname(lib), "-lrna4r", "-Wl,-rpath," + os.path.dirname(lib)])
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
+    assert "c_abi_check ok" in out.stdout
+
+
 def test_strerror_and_version_need_no_gpu():
     from paper_1307_7820_b200 import load
     L = load()
@@ -42,7 +56,7 @@ def test_prepare_rejects_bad_q_and_null_before_touching_cuda():
     assert L.rna4r_prepare(13, 0, None, ctypes.byref(h)) == -1
     assert L.rna4r_prepare(8, 0, None, None) == -2
     assert L.rna4r_destroy(None) == -5
-    assert L.rna4r_workspace_bytes(None, 10, 1) == 0
+    assert L.rna4r_workspace_bytes(None, 10, 1, 0) == 0
 
 
 def test_no_cpu_fallback_without_gpu():

@@ -195,6 +195,18 @@ def test_cfg3_n6000_q8(rna):
     check_large(rna, "cfg3", 8, rna.ENGINE_TILED)
 
 
+def test_cfg3_full_table_elementwise(rna):
+    """the whole 6000 x 6000 table, element by element, against the oracle's table (not only samples and sums)"""
+    s = workloads.single_config("cfg3")
+    res = oracle.nussinov_fast(s, threads=os.cpu_count() or 1, want_table=True)
+    r = ctx(rna, 8, rna.ENGINE_TILED)
+    score, tab = r.fold(dev_seq(s), len(s), table_dtype=rna.TABLE_INT16)
+    torch.cuda.synchronize()
+    assert int(score.item()) == res["score"] == 2761
+    want = torch.from_numpy(np.ascontiguousarray(res["table"]).astype(np.int16)).cuda()
+    assert torch.equal(tab, want), int((tab != want).sum().item())
+
+
 def test_cfg3_n6000_q8_diag_engine(rna):
     check_large(rna, "cfg3", 8, rna.ENGINE_DIAG)
 
