@@ -76,12 +76,17 @@ extern "C" {
 #define RNA4R_TABLE_INT32  2
 
 /* ---- fill engines ---- */
-#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 10, else DIAG                         */
+#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 10, else DIAG; rna4r_fold_batch takes SMEM when
+                                     4 <= q <= 8 and every sequence is <= rna4r_smem_max_n(ctx)  */
 #define RNA4R_ENGINE_TILED  1     /* persistent super-tile wavefront, R resident in shared memory
                                      (the B200 design)                     */
 #define RNA4R_ENGINE_DIAG   2     /* paper-literal section 4 algorithm: one launch per anti-
                                      diagonal, one thread per cell, per-cell sliding vectors
                                      (PAPER.md:249-267); any q in 2..12; the comparison point   */
+
+#define RNA4R_ENGINE_SMEM   3     /* one CTA per sequence, the whole fold's row / column words resident
+                                     in shared memory (batches of short sequences, BASELINE.json
+                                     configs[3]); q in 4..8, n <= rna4r_smem_max_n */
 
 typedef struct rna4r_ctx rna4r_ctx;   /* opaque; owns the device R tables for one q on one device */
 
@@ -117,6 +122,9 @@ int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact);
 /* Selects the fill engine (RNA4R_ENGINE_*) for later fold calls.  Errors: CONTEXT, ENGINE. */
 int rna4r_set_engine(rna4r_ctx *ctx, int engine);
 int rna4r_engine(const rna4r_ctx *ctx);   /* the engine fold calls will use (resolved, never AUTO) */
+/* Longest sequence RNA4R_ENGINE_SMEM folds for the context's q (its state has to fit 227 KB of shared memory),
+ * -1 if the engine does not support this q, or RNA4R_ERR_CONTEXT. */
+int rna4r_smem_max_n(const rna4r_ctx *ctx);
 
 /*
  * Workspace size in bytes for `count` sequences each of length <= n_max with the context's current

@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 TABLE_NONE, TABLE_INT16, TABLE_INT32 = 0, 1, 2
-ENGINE_AUTO, ENGINE_TILED, ENGINE_DIAG = 0, 1, 2
+ENGINE_AUTO, ENGINE_TILED, ENGINE_DIAG, ENGINE_SMEM = 0, 1, 2, 3
 
 _lib = None
 
@@ -49,6 +49,7 @@ def load():
     L.rna4r_table_to_host.argtypes = [vp, vp, ctypes.c_int]
     L.rna4r_set_engine.argtypes = [vp, ctypes.c_int]
     L.rna4r_engine.argtypes = [vp]
+    L.rna4r_smem_max_n.argtypes = [vp]
     L.rna4r_workspace_bytes.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int]
     L.rna4r_set_max_blocks_per_sm.argtypes = [vp, ctypes.c_int]
     L.rna4r_set_max_blocks.argtypes = [vp, ctypes.c_int]
@@ -125,6 +126,10 @@ class Rna4r:
     @property
     def engine(self) -> int:
         return self.lib.rna4r_engine(self.h)
+
+    def smem_max_n(self) -> int:
+        """rna4r_smem_max_n: longest sequence ENGINE_SMEM folds at this q (-1: q not supported)."""
+        return self.lib.rna4r_smem_max_n(self.h)
 
     def table(self) -> np.ndarray:
         """R as a numpy uint8 array [2^q, 2^q] (host copy via rna4r_table_to_host)."""

@@ -1,18 +1,31 @@
 // api.cu -- the C ABI of librna4r.so (include/rna4r.h): context, workspace planning, dispatch.
+#include <new>
 #include "common.cuh"
 #include "rtable.cuh"
 #include "diag_engine.cuh"
 #include "tiled_engine.cuh"
+#include "smem_engine.cuh"
 #include "traceback.cuh"
 #include "microbench.cuh"
 
-#include <new>
 
 namespace {
 
 constexpr int kDelta = 0;   // 0: the tiled engine picks the product-stage span from the problem size
 
 inline bool ctx_ok(const rna4r_ctx *c) { return c && c->magic == RNA4R_MAGIC; }
+
+template <typename F>
+auto dispatch_q_smem(int q, F &&f) -> decltype(f(std::integral_constant<int, 8>{}))
+{
+    switch (q) {
+    case 4: return f(std::integral_constant<int, 4>{});
+    case 5: return f(std::integral_constant<int, 5>{});
+    case 6: return f(std::integral_constant<int, 6>{});
+    case 7: return f(std::integral_constant<int, 7>{});
+    default: return f(std::integral_constant<int, 8>{});
+    }
+}
 
 template <typename F>
 auto dispatch_q(int q, F &&f) -> decltype(f(std::integral_constant<int, 8>{}))
@@ -45,8 +58,23 @@ size_t tiled_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_sing
     return dispatch_q(ctx->q, [&](auto Q) { return tiled::workspace_bytes_q<decltype(Q)::value>(kDelta, lens, count, n_single); });
 }
 
+// RNA4R_ENGINE_SMEM: q = 4..8, and the sequence's state has to fit one CTA's shared memory (n <= 704 at q = 8)
+inline bool smem_q_ok(int q) { return q >= 4 && q <= 8; }
+inline int smem_max_n(int q)
+{
+    switch (q) {
+    case 4: return smemseq::max_n<4>();
+    case 5: return smemseq::max_n<5>();
+    case 6: return smemseq::max_n<6>();
+    case 7: return smemseq::max_n<7>();
+    case 8: return smemseq::max_n<8>();
+    default: return -1;
+    }
+}
+
 size_t engine_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_single)
 {
+    if (ctx->engine == RNA4R_ENGINE_SMEM) return smemseq::workspace_bytes(count);
     if (ctx->engine == RNA4R_ENGINE_TILED) return tiled_ws(ctx, lens, count, n_single);
     // DIAG: sequences of a batch are folded one after another, each in its own slice
     size_t total = 0;
@@ -58,6 +86,7 @@ int check_n(const rna4r_ctx *ctx, int n)
 {
     if (n < 0 || n > 65534) return RNA4R_ERR_BAD_N;
     if (ctx->engine == RNA4R_ENGINE_TILED && n > tiled_max_n(ctx->q)) return RNA4R_ERR_BAD_N;
+    if (ctx->engine == RNA4R_ENGINE_SMEM && n > smem_max_n(ctx->q)) return RNA4R_ERR_BAD_N;
     return RNA4R_OK;
 }
 
@@ -106,6 +135,7 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0; ctx->max_blocks_per_sm = 0; ctx->max_blocks = 0;
     ctx->timing = 0; ctx->timing_valid = 0; ctx->ev0 = ctx->ev1 = nullptr;
     ctx->trace = nullptr; ctx->trace_tiles = 0;
+    ctx->engine_auto = 1; ctx->order_host = nullptr; ctx->order_cap = 0;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t N = (size_t)1 << q, M = (size_t)1 << (q - 1);
     auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4); delete ctx; return RNA4R_ERR_CUDA; };
@@ -139,6 +169,7 @@ int rna4r_destroy(rna4r_ctx *ctx)
     cudaFree(ctx->trace);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    delete[] ctx->order_host;
     ctx->magic = 0;
     delete ctx;
     return RNA4R_OK;
@@ -148,6 +179,7 @@ int rna4r_q(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->q : RNA4R_ERR_CONT
 const uint8_t *rna4r_table(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->R : nullptr; }
 const uint8_t *rna4r_table_compact(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->Rc : nullptr; }
 int rna4r_engine(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->engine : RNA4R_ERR_CONTEXT; }
+int rna4r_smem_max_n(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? smem_max_n(ctx->q) : RNA4R_ERR_CONTEXT; }
 int rna4r_last_launch_count(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->last_launches : RNA4R_ERR_CONTEXT; }
 int rna4r_last_cuda_error(const rna4r_ctx *ctx) { return ctx_ok(ctx) ? ctx->last_cuda_error : RNA4R_ERR_CONTEXT; }
 
@@ -214,10 +246,13 @@ int rna4r_last_fill_kernel_ms(rna4r_ctx *ctx, float *ms_host)
 int rna4r_set_engine(rna4r_ctx *ctx, int engine)
 {
     if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
-    if (engine == RNA4R_ENGINE_AUTO) engine = (ctx->q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
-    if (engine != RNA4R_ENGINE_TILED && engine != RNA4R_ENGINE_DIAG) return RNA4R_ERR_ENGINE;
+    const int is_auto = engine == RNA4R_ENGINE_AUTO;
+    if (is_auto) engine = (ctx->q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
+    if (engine != RNA4R_ENGINE_TILED && engine != RNA4R_ENGINE_DIAG && engine != RNA4R_ENGINE_SMEM) return RNA4R_ERR_ENGINE;
     if (engine == RNA4R_ENGINE_TILED && ctx->q > 10) return RNA4R_ERR_ENGINE;
+    if (engine == RNA4R_ENGINE_SMEM && !smem_q_ok(ctx->q)) return RNA4R_ERR_ENGINE;
     ctx->engine = engine;
+    ctx->engine_auto = is_auto;
     return RNA4R_OK;
 }
 
@@ -247,6 +282,7 @@ size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count, int fla
     if (count > 0) {
         // every sequence at n_max: per-sequence cost is monotone in n
         if (ctx->engine == RNA4R_ENGINE_TILED) core = (size_t)count * tiled_ws(ctx, nullptr, 1, n_max);
+        else if (ctx->engine == RNA4R_ENGINE_SMEM) core = smemseq::workspace_bytes(count);
         else core = (size_t)count * diag_ws_layout(nullptr, n_max).bytes;
     }
     if (!(flags & (RNA4R_WS_HOST_STAGING | RNA4R_WS_HOST_TABLE16 | RNA4R_WS_HOST_TABLE32))) return core;
@@ -282,6 +318,11 @@ int rna4r_fold(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_out
         const size_t es = table_dtype == RNA4R_TABLE_INT16 ? 2 : 4;
         RNA4R_CUDA(ctx, cudaMemsetAsync(table_out_dev, 0, (size_t)n * n * es, st));   // zeros below the diagonal
     }
+    if (ctx->engine == RNA4R_ENGINE_SMEM)
+        return dispatch_q_smem(ctx->q, [&](auto Q) {
+            return smemseq::enqueue_q<decltype(Q)::value>(ctx, seq_dev, nullptr, nullptr, 1, n, score_out_dev, nullptr, table_out_dev,
+                                                          table_dtype, workspace_dev, st);
+        });
     return dispatch_q(ctx->q, [&](auto Q) {
         return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seq_dev, nullptr, nullptr, 1, n, score_out_dev, nullptr,
                                                     table_out_dev, table_dtype, workspace_dev, st);
@@ -327,6 +368,19 @@ int rna4r_fold_batch_status(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64
         ctx->last_launches = launches;
         return RNA4R_OK;
     }
+    // Batches of short sequences go to the CTA-per-sequence engine when the engine was left on AUTO:
+    // every sequence's state has to fit one CTA's shared memory; otherwise the whole batch runs on the tiled engine.
+    bool use_smem = ctx->engine == RNA4R_ENGINE_SMEM;
+    if (!use_smem && ctx->engine_auto && smem_q_ok(ctx->q)) {
+        const int lim = smem_max_n(ctx->q);
+        use_smem = true;
+        for (int t = 0; t < count; ++t) if (lens_host[t] > lim) { use_smem = false; break; }
+    }
+    if (use_smem)
+        return dispatch_q_smem(ctx->q, [&](auto Q) {
+            return smemseq::enqueue_q<decltype(Q)::value>(ctx, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
+                                                          status_out_dev, nullptr, RNA4R_TABLE_NONE, workspace_dev, st);
+        });
     return dispatch_q(ctx->q, [&](auto Q) {
         return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
                                                     status_out_dev, nullptr, RNA4R_TABLE_NONE, workspace_dev, st);

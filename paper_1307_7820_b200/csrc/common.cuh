@@ -24,6 +24,9 @@ struct rna4r_ctx {
     cudaEvent_t ev0, ev1;
     unsigned long long *trace;   // optional per-super-tile phase stamps (rna4r_set_trace)
     int trace_tiles;
+    int engine_auto;         // the engine was left on (or set back to) RNA4R_ENGINE_AUTO: batches of short sequences take the SMEM engine
+    int32_t *order_host;     // host scratch of the SMEM engine: sequence indices sorted by length (grown on demand)
+    int order_cap;
 };
 // u64 words per super-tile in the optional trace buffer (rna4r_set_trace); a build with
 // -DRNA4R_TRACE_WORDS=256 adds per-q-tile event stamps for tuning

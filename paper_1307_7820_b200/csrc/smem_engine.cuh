@@ -1,0 +1,578 @@
+// smem_engine.cuh -- RNA4R_ENGINE_SMEM: one CTA per sequence, the whole fold resident in shared memory.
+//
+// The engine for batches of short sequences (BASELINE.json configs[3]; north_star "batch many sequences to fill the
+// machine on short diagonals").  Same coordinates and the same two-vector step as
+// tiled_engine.cuh: M(r,c) = D(r+1,c), group g = split indices t in [gq, gq+q), and for row r, column c
+//     max_{t in g} M(r,t) + M(t,c) = M(r,gq) + M(gq,c) + Rc[h][v]                     (eq. (3))
+// with h / v the q-1 informative difference bits of the row run / the column run (v_0 = 0).
+//
+// What is stored ("only the horizontal and vertical differences are stored", plus anchors, reading g21):
+//   W[g][r]  (r < gq)   row word of row r over group g, 32 bit:  h << 24 | M(r,gq)
+//   X[g][c]  (c >= gq)  column word of column c over group g, 16 bit:  v << (16-HB) | M(gq,c); expanded on load to
+//                       v << (24-HB) | M(gq,c), so that S = W + X has the table index h*2^HB + v at bit 24-HB and
+//                       the anchor sum in the low halfword: one lookup = add, LEA.HI, LDS.U8, VIADDMNMX.U16x2.
+// Nothing else of the table is kept: n^2/(2q) words of each kind (n = 700, q = 8: 122 KB + 61 KB).
+//
+// Schedule.  q x q tiles (A,B); the tiles of one tile-diagonal D = B - A are independent.  For a tile
+// the groups strictly between A and B are complete for all its q^2 cells (Alg. 1 lines 15-19);
+// groups A and B are the paper's residual loops.  Per tile-diagonal step D, one CTA barrier apart:
+//   phase A   (i) waves: the closure of every tile of diagonal D, 4 tiles per warp (Q lanes each), and
+//             (ii) "early bulk" of diagonal D+1: for every strip-tile (tile-row A x 4 tile-columns = 32 columns) whose
+//             first tile lies on diagonal D+1, the complete groups that no tile of diagonal D feeds -- lanes <-> 32
+//             columns of ONE row, so the row word is warp-uniform and the table gather is conflict-free;
+//   phase B   the groups of those strip-tiles that diagonal D completed; the maxima are packed into one word per
+//             column (value of the bottom row + 3-bit offsets of the rows above: Lemma 1 bounds them by q-1).
+// The few groups a strip-tile cannot take for its 2nd..4th tile column ("fresh" groups, at most 3 per side) are
+// looked up inside the wave.
+//
+// Wave of tile (A,B), row-parallel: rows from the bottom up, the Q cells of a row at once.  With
+//   C'(a,y) = max{ bulk, b + M(r+1,c-1), head: max_{t in group A, t>r} M(r,t)+M(t,c) }   -- rows below only
+// the row is  V(a,y) = max_{y' <= y} C'(a,y') + Qd(y',y),  Qd = the diagonal tile (B,B): the in-row dependency
+// V(a,y) >= V(a,y') + Qd(y',y) collapses because Qd is superadditive (M(i,k) >= M(i,j) + M(j,k)).  The head is one
+// masked lookup with the running column word; the tail is a max-plus over the row's packed C' values
+// (4 DPX VIADDMNMX.S16x2).  No skewed wavefront: 8 dependent steps per tile, every lane busy in every step.
+#pragma once
+#include "common.cuh"
+
+namespace smemseq {
+
+template <int Q>
+struct Cfg {
+    static_assert(Q >= 4 && Q <= 8, "the shared-memory engine is built for q = 4..8");
+    static constexpr int HB = Q - 1;                 // informative bits per vector
+    static constexpr int G = 4;                      // q-tiles per warp and per column strip
+    static constexpr int SW = G * Q;                 // strip width in columns (<= 32)
+    static constexpr int ISH = 24 - HB;              // position of the table index in a word sum
+    static constexpr int XAB = 16 - HB;              // anchor bits of a stored column word
+    static constexpr uint32_t XAMASK = (1u << XAB) - 1u;
+    static constexpr uint32_t XMUL = (1u << ISH) - (1u << XAB);
+    static constexpr uint32_t HMASK = (1u << HB) - 1u;
+    static constexpr int TBL_BYTES = 1 << (2 * HB);
+    static constexpr int TBL_AREA = TBL_BYTES < 256 ? 256 : TBL_BYTES;
+    static constexpr int NWARP = 24;
+    static constexpr int NTHR = NWARP * 32;
+    static constexpr int NP = (Q + 1) / 2;           // packed value pairs of a tile row
+    static constexpr int NF = G - 1;                 // fresh groups per side
+    static constexpr int PB_SLOTS = 32;              // partial-maximum rows between phase A and phase B
+    static constexpr int VBITS = 11;                 // value bits of a packed bulk word (D <= 2047)
+    static constexpr int SCR_BYTES = NWARP * 2 * G * 16;   // per-warp row scratch: [2][G] x 8 halfwords
+    static constexpr int FIXED_BYTES = TBL_AREA + SCR_BYTES + 64;
+    static constexpr int MAX_SMEM = 232448;          // 227 KB
+};
+
+// byte offsets of one sequence's state, relative to the start of the pool
+struct Layout {
+    int NB;
+    uint32_t W, X, val, wdh, dq, pm, rl, code, part, total;
+};
+
+template <int Q>
+__host__ __device__ inline Layout make_layout(int n)
+{
+    Layout L;
+    const uint32_t NB = (uint32_t)(n / Q + 1);
+    L.NB = (int)NB;
+    uint32_t off = 0;
+    auto take = [&](uint32_t bytes) { const uint32_t o = off; off += (bytes + 15u) & ~15u; return o; };
+    L.W = take(4u * Q * NB * (NB - 1) / 2);
+    L.X = take(2u * Q * NB * (NB + 1) / 2);
+    L.val = take(4u * 32u * NB);
+    L.wdh = take(4u * Q * NB);
+    L.dq = take(8u * Q * NB);
+    L.pm = take(4u * NB);
+    L.rl = take(2u * Q * NB);
+    L.code = take(Q * NB + 16u);
+    L.part = take(4u * 32u * Cfg<Q>::PB_SLOTS);
+    L.total = off;
+    return L;
+}
+
+// largest n this engine folds: the state has to fit the pool, the anchors their fields
+template <int Q>
+inline int max_n()
+{
+    const uint32_t pool = (uint32_t)(Cfg<Q>::MAX_SMEM - Cfg<Q>::FIXED_BYTES);
+    int lim = 2 * ((1 << Cfg<Q>::XAB) - 1);                         // D <= n/2 < 2^XAB
+    if (lim > 2 * ((1 << Cfg<Q>::VBITS) - 1)) lim = 2 * ((1 << Cfg<Q>::VBITS) - 1);
+    int lo = 0, hi = lim;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) / 2;
+        if (make_layout<Q>(mid).total <= pool) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+struct Params {
+    const uint8_t *seqs;
+    const int64_t *offsets;   // device [count+1], or NULL for a single sequence of length n_single
+    const int32_t *lens;      // device [count] (batch only)
+    const int32_t *order;     // device [grid]: sequence folded by CTA b (longest first), or NULL: CTA b folds b
+    int n_single;
+    const uint8_t *tbl;       // compact table Rc, bytes, natural pitch
+    int32_t *scores;
+    int32_t *status;          // NULL or [count]
+    void *table_out;          // NULL, or n*n elements (single sequence only)
+    int table_dtype;
+};
+
+template <int Q>
+struct Sm {
+    uint32_t tbl_sa;          // shared-space address of the table
+    uint16_t *scr;            // per-warp row scratch
+    int *misc;                // [0] task counter, [1] invalid flag
+    uint32_t *W;
+    uint16_t *X;
+    uint32_t *val;
+    uint32_t *wdh;
+    uint8_t *dq;
+    uint8_t *pm;
+    int16_t *rl;
+    int8_t *code;
+    uint32_t *part;
+    int n, NB;
+};
+
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// acc = max(acc, candidate of the word sum S): eq. (3).  No mask on the index: a don't-care S of an
+// idle lane indexes at most 2^(8+HB) bytes past the table, inside the CTA's window (the pool follows the table).
+template <int Q>
+__device__ __forceinline__ uint32_t lookup_max(uint32_t tbl_sa, uint32_t S, uint32_t acc)
+{
+    uint32_t rv;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"((S >> Cfg<Q>::ISH) + tbl_sa));
+    return __viaddmax_u16x2(S, rv, acc);
+}
+
+template <int Q>
+__device__ __forceinline__ uint32_t expand_x(uint32_t x16) { return x16 + (x16 >> Cfg<Q>::XAB) * Cfg<Q>::XMUL; }
+
+template <int Q> __device__ __forceinline__ int off_w(int g) { return Q * (g * (g - 1) / 2); }                 // words
+template <int Q> __device__ __forceinline__ int off_x(int NB, int g) { return Q * (g * NB - g * (g - 1) / 2); } // halfwords
+
+// step a8 for the test / inspection path: out[(i-1)*n + (j-1)] = D(i,j) = M(i-1, j)
+template <bool TABLE>
+__device__ __forceinline__ void store_cell(const Params &p, int n, int r, int c, int v)
+{
+    if constexpr (TABLE) {
+        if (r < n && c >= r + 1 && c <= n) {
+            if (p.table_dtype == RNA4R_TABLE_INT16) reinterpret_cast<int16_t *>(p.table_out)[(size_t)r * n + c - 1] = (int16_t)v;
+            else reinterpret_cast<int32_t *>(p.table_out)[(size_t)r * n + c - 1] = v;
+        }
+    }
+}
+
+// ---- bulk (step a4): rows of tile-row A x the 32 columns of a strip, groups glo..ghi --------------------------------
+// lane <-> column cx, a thread owns the Q rows; the row words are warp-uniform (broadcast loads), so all 32 gathers
+// of a lookup fall in one table row: conflict-free.
+template <int Q>
+__device__ __forceinline__ void strip_groups(const Sm<Q> &s, int A, int cx, int glo, int ghi, uint32_t (&acc)[Q])
+{
+    const uint32_t *w = s.W + off_w<Q>(glo) + A * Q;
+    const uint16_t *x = s.X + off_x<Q>(s.NB, glo) - glo * Q + cx;
+#pragma unroll 2
+    for (int g = glo; g <= ghi; ++g) {
+        const uint32_t X32 = expand_x<Q>(*x);
+        uint32_t wr[Q];
+        if constexpr (Q % 4 == 0) {
+#pragma unroll
+            for (int i = 0; i < Q / 4; ++i) {
+                const uint4 t = reinterpret_cast<const uint4 *>(w)[i];
+                wr[4 * i] = t.x; wr[4 * i + 1] = t.y; wr[4 * i + 2] = t.z; wr[4 * i + 3] = t.w;
+            }
+        } else {
+#pragma unroll
+            for (int a = 0; a < Q; ++a) wr[a] = w[a];
+        }
+#pragma unroll
+        for (int a = 0; a < Q; ++a) acc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, acc[a]);
+        w += Q * g;
+        x += Q * (s.NB - g - 1);
+    }
+}
+
+// Bulk maxima of one column, packed: value of the bottom row | 3-bit offsets of the rows above.  All candidates of a
+// strip-tile range over the same splits t, and M(r,t) - M(r_bottom,t) lies in [0, Q-1] (Lemma 1), so
+// the maxima of the rows differ from the bottom row's by 0..Q-1.
+template <int Q>
+__device__ __forceinline__ uint32_t pack_rows(const uint32_t (&acc)[Q])
+{
+    const uint32_t base = acc[Q - 1] & 0xffffu;
+    uint32_t w = base;
+#pragma unroll
+    for (int a = 0; a < Q - 1; ++a) w |= (((acc[a] & 0xffffu) - base) & 7u) << (Cfg<Q>::VBITS + 3 * a);
+    return w;
+}
+template <int Q>
+__device__ __forceinline__ int unpack_row(uint32_t w, int a)
+{
+    const int base = (int)(w & ((1u << Cfg<Q>::VBITS) - 1u));
+    return a == Q - 1 ? base : base + (int)((w >> (Cfg<Q>::VBITS + 3 * a)) & 7u);
+}
+
+// ---- diagonal tile (A,A): plain eq. (1) on Q x Q cells, one thread --------------------------------------------------
+template <int Q, bool TABLE>
+__device__ void diag_tile(const Params &p, const Sm<Q> &s, int seq, int A)
+{
+    using C = Cfg<Q>;
+    const int r0 = A * Q;
+    int m[Q][Q];
+    int cd[Q];
+#pragma unroll
+    for (int a = 0; a < Q; ++a) {
+        cd[a] = s.code[r0 + a];
+#pragma unroll
+        for (int y = 0; y < Q; ++y) m[a][y] = 0;
+    }
+#pragma unroll
+    for (int d = 2; d < Q; ++d) {
+#pragma unroll
+        for (int a = 0; a + d < Q; ++a) {
+            const int y = a + d;
+            int best = m[a + 1][y - 1] + rna4r_pair(cd[a], cd[y - 1]);      // b(S_i,S_j) + D(i+1,j-1)
+#pragma unroll
+            for (int t = a + 1; t < y; ++t) best = max(best, m[a][t] + m[t][y]);
+            m[a][y] = best;
+        }
+    }
+    uint16_t *xo = s.X + off_x<Q>(s.NB, A);
+#pragma unroll
+    for (int y = 0; y < Q; ++y) {
+        uint32_t vb = 0;
+#pragma unroll
+        for (int j = 1; j < Q; ++j) vb |= (uint32_t)(m[j - 1][y] - m[j][y]) << (j - 1);
+        xo[y] = (uint16_t)((vb << C::XAB) | (uint32_t)m[0][y]);
+        uint8_t *dq = s.dq + (size_t)(r0 + y) * 8;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) dq[t] = (t < Q && t < y) ? (uint8_t)m[t][y] : (uint8_t)0;
+    }
+#pragma unroll
+    for (int a = 0; a < Q; ++a) {
+        uint32_t hb = 0;
+#pragma unroll
+        for (int j = 1; j < Q; ++j) hb |= (uint32_t)(m[a][j] - m[a][j - 1]) << (j - 1);
+        s.wdh[r0 + a] = hb << 24;
+        s.rl[r0 + a] = (int16_t)m[a][Q - 1];
+        if constexpr (TABLE) {
+#pragma unroll
+            for (int y = 0; y < Q; ++y) store_cell<TABLE>(p, s.n, r0 + a, r0 + y, m[a][y]);
+        }
+    }
+    if (A == 0 && s.n < Q) {
+        int v = 0;
+#pragma unroll
+        for (int y = 0; y < Q; ++y) if (y == s.n) v = m[0][y];
+        p.scores[seq] = v;                                                   // M(0,n) = D(1,n)
+    }
+}
+
+// ---- wave: closure of up to G tiles of tile-diagonal D, residue class rho = A mod G, task jt ------------------------
+template <int Q, bool TABLE>
+__device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int seq, int D, int rho, int jt, int warp, int lane)
+{
+    using C = Cfg<Q>;
+    constexpr uint32_t FULL = 0xffffffffu;
+    const int NB = s.NB, NT = NB - D;
+    const bool lane_ok = lane < C::SW;
+    const int i = lane_ok ? lane / Q : C::G - 1;
+    const int y = lane_ok ? lane - i * Q : Q - 1;
+    const int cnt = (NT - rho + C::G - 1) / C::G;              // tiles of this residue class on the diagonal
+    int j = jt * C::G + i;
+    const bool own = lane_ok && j < cnt;
+    if (j >= cnt) j = jt * C::G;                               // shadow of the first tile: computes, stores nothing
+    const int A = rho + C::G * j, B = A + D;
+    const int k = B % C::G, GC = B - k, D0 = D - k;            // k, D0: the same for every tile of the task
+    const int r0 = A * Q, c = B * Q + y;
+
+    // bulk maxima of the strip-tile (phase B of step D0 - 1); none before the strip-tile's first diagonal is 2
+    uint32_t vw = 0;
+    if (D0 >= 2) vw = s.val[A * 32 + k * Q + y];
+    // fresh groups: head side A+1 .. A+nfh (column words of the tiles below), tail side GC .. GC+nft-1 (row words of
+    // the tiles to the left inside the strip).  Without bulk (D0 < 2) the D-1 complete groups are all fresh.
+    const int nfh = (D0 >= 2) ? k : D - 1;
+    const int nft = (D0 >= 2) ? k : 0;
+    uint32_t Xf[2 * C::NF];
+    const uint32_t *Wf[2 * C::NF];
+#pragma unroll
+    for (int t = 0; t < C::NF; ++t) {
+        Xf[t] = 0; Wf[t] = s.W;
+        if (t < nfh) {
+            const int g = A + 1 + t;
+            Xf[t] = expand_x<Q>(s.X[off_x<Q>(NB, g) + c - g * Q]);
+            Wf[t] = s.W + off_w<Q>(g) + r0;
+        }
+        Xf[C::NF + t] = 0; Wf[C::NF + t] = s.W;
+        if (t < nft) {
+            const int g = GC + t;
+            Xf[C::NF + t] = expand_x<Q>(s.X[off_x<Q>(NB, g) + c - g * Q]);
+            Wf[C::NF + t] = s.W + off_w<Q>(g) + r0;
+        }
+    }
+    // diagonal tile (B,B) for the tail: packed pairs (Qd(2j,y), Qd(2j+1,y)); y' > y is "minus infinity"
+    int Qp[C::NP];
+    {
+        const uint2 qb = *reinterpret_cast<const uint2 *>(s.dq + (size_t)c * 8);
+#pragma unroll
+        for (int jj = 0; jj < C::NP; ++jj) {
+            const uint32_t src = jj < 2 ? qb.x : qb.y;
+            uint32_t pr = __byte_perm(src, 0, (jj & 1) ? 0x4342 : 0x4140);
+            if (2 * jj > y) pr |= 0x8000u;
+            if (2 * jj + 1 > y) pr |= 0x80000000u;
+            Qp[jj] = (int)pr;
+        }
+    }
+    // pairing mask of my column against the rows of the tile-row: bit a <-> b(S[r0+a], S[c-1])
+    uint32_t pm = 0;
+    {
+        const int cc = s.code[c - 1];
+        if (cc < 4) pm = s.pm[A * 4 + cc];
+    }
+    // bottom edge M((A+1)q, c): anchor of the column word of group A+1; left column M(r0+1+y, Bq-1) for lane 0's
+    // pair term: the last value tile (A,B-1) left in its rows, and for the row below the tile an anchor again
+    const uint16_t *xbelow = s.X + off_x<Q>(NB, A + 1) - (A + 1) * Q;
+    int vprev = (int)(xbelow[c] & C::XAMASK);
+    int Lc;
+    if (y < Q - 1) Lc = s.rl[r0 + 1 + y];
+    else Lc = (D >= 2) ? (int)(xbelow[B * Q - 1] & C::XAMASK) : 0;
+    const uint32_t *wh = s.wdh + r0;
+    uint16_t *scr = s.scr + (size_t)warp * (2 * C::G * 8);
+    uint32_t *wout = s.W + off_w<Q>(B) + r0;
+    uint32_t xbits = 0;
+    uint32_t Xp = (uint32_t)vprev;
+    int vl = __shfl_sync(FULL, vprev, lane - 1);                  // M(r+1, c-1) for the bottom row
+    int v = 0;
+#pragma unroll
+    for (int a = Q - 1; a >= 0; --a) {
+        // ---- candidates from the rows below: bulk, pair term (a3), head residual (a5), fresh groups (a4)
+        const int lca = __shfl_sync(FULL, Lc, i * Q + a);
+        const int vd = (y == 0) ? lca : vl;
+        int cand = unpack_row<Q>(vw, a);
+        cand = max(cand, vd + (int)((pm >> a) & 1u));
+        uint32_t best = lookup_max<Q>(s.tbl_sa, wh[a] + Xp, (uint32_t)cand);
+#pragma unroll
+        for (int t = 0; t < 2 * C::NF; ++t) {
+            const bool on = (t < C::NF) ? (t < nfh) : (t - C::NF < nft);          // warp-uniform
+            if (on) best = lookup_max<Q>(s.tbl_sa, Wf[t][a] + Xf[t], best);
+        }
+        // ---- tail: V(a,y) = max_{y' <= y} C'(a,y') + Qd(y',y)
+        uint16_t *row = scr + ((a & 1) * C::G + i) * 8;
+        if (lane_ok) row[y] = (uint16_t)(best & 0xffffu);
+        __syncwarp();
+        int m2 = (int)0x80008000u;
+        if constexpr (Q == 8) {
+            const uint4 t4 = *reinterpret_cast<const uint4 *>(row);
+            const int m3 = __viaddmax_s16x2((int)t4.x, Qp[0], m2);
+            const int m4 = __viaddmax_s16x2((int)t4.y, Qp[1], m2);
+            const int m5 = __viaddmax_s16x2((int)t4.z, Qp[2], m3);
+            const int m6 = __viaddmax_s16x2((int)t4.w, Qp[3], m4);
+            m2 = __vmaxs2(m5, m6);
+        } else {
+#pragma unroll
+            for (int jj = 0; jj < C::NP; ++jj) m2 = __viaddmax_s16x2((int)reinterpret_cast<const uint32_t *>(row)[jj], Qp[jj], m2);
+        }
+        v = max((int)(short)(m2 & 0xffff), m2 >> 16);
+        // ---- step a6: row word of row r over group B (ballot of the horizontal differences), column word bit
+        vl = __shfl_sync(FULL, v, lane - 1);
+        const uint32_t bal = __ballot_sync(FULL, y > 0 && v != vl);
+        if (own && y == 0) wout[a] = (((bal >> (i * Q + 1)) & C::HMASK) << 24) | (uint32_t)v;
+        if (own && y == Q - 1) s.rl[r0 + a] = (int16_t)v;
+        if (a < Q - 1) xbits |= (uint32_t)(v - vprev) << (C::ISH + a);
+        Xp = xbits | (uint32_t)v;
+        vprev = v;
+        if (own) store_cell<TABLE>(p, s.n, r0 + a, c, v);
+    }
+    if (own) {
+        s.X[off_x<Q>(NB, A) + c - A * Q] = (uint16_t)(((xbits >> C::ISH) << C::XAB) | (uint32_t)v);
+        if (A == 0 && c == s.n) p.scores[seq] = v;                // M(0,n) = D(1,n)
+    }
+}
+
+// strip-tiles whose first tile lies on diagonal D0: A = Afirst + G*i, i < nE
+__device__ __forceinline__ void strips_of(int NB, int G, int D0, int &Afirst, int &nE)
+{
+    Afirst = (G - D0 % G) % G;
+    nE = (D0 < NB && NB - 1 - D0 >= Afirst) ? (NB - 1 - D0 - Afirst) / G + 1 : 0;
+}
+
+template <int Q, bool TABLE>
+__global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
+{
+    using C = Cfg<Q>;
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int seq = p.order ? p.order[blockIdx.x] : (int)blockIdx.x;
+    const int n = p.offsets ? p.lens[seq] : p.n_single;
+    const Layout L = make_layout<Q>(n);
+    Sm<Q> s;
+    {
+        uint8_t *b = smem_raw;
+        s.tbl_sa = smem_addr(b); b += C::TBL_AREA;
+        s.scr = (uint16_t *)b; b += C::SCR_BYTES;
+        s.misc = (int *)b; b += 64;
+        s.W = (uint32_t *)(b + L.W); s.X = (uint16_t *)(b + L.X); s.val = (uint32_t *)(b + L.val);
+        s.wdh = (uint32_t *)(b + L.wdh); s.dq = b + L.dq; s.pm = b + L.pm; s.rl = (int16_t *)(b + L.rl);
+        s.code = (int8_t *)(b + L.code); s.part = (uint32_t *)(b + L.part);
+        s.n = n; s.NB = L.NB;
+        uint32_t dyn;
+        asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+        if ((uint32_t)C::FIXED_BYTES + L.total > dyn) __trap();       // the host routes longer sequences elsewhere: fail loudly
+    }
+    const int NB = s.NB;
+    // ---- setup: table, codes (step a1), zeroed column words (an unwritten word is a valid lower bound)
+    {
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(p.tbl);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(smem_raw);
+        for (int e = tid; e < C::TBL_BYTES / 4; e += C::NTHR) dst[e] = __ldg(src + e);
+        for (int e = tid; e < C::SCR_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(s.scr)[e] = 0;
+        if (tid < 16) s.misc[tid] = 0;
+    }
+    __syncthreads();
+    {
+        int bad = 0;
+        if (p.offsets && p.offsets[seq + 1] - p.offsets[seq] != (int64_t)n) bad = RNA4R_STATUS_BAD_OFFSETS;
+        const uint8_t *src = p.seqs + (p.offsets && !bad ? p.offsets[seq] : 0);
+        for (int x = tid; x < NB * Q + 16; x += C::NTHR) {
+            int cde = 4;
+            if (x < n && !bad) { cde = rna4r_base_code(src[x]); if (cde == 4) bad |= RNA4R_STATUS_BAD_BASE; }
+            s.code[x] = (int8_t)cde;
+        }
+        if (bad) atomicOr(&s.misc[1], bad);
+        uint4 *xz = reinterpret_cast<uint4 *>(s.X);
+        const int nx = (int)((L.val - L.X) / 16);
+        for (int e = tid; e < nx; e += C::NTHR) xz[e] = make_uint4(0, 0, 0, 0);
+    }
+    __syncthreads();
+    if (s.misc[1]) {                                   // reading g4: not a base -> score -1, status word
+        if (tid == 0) { p.scores[seq] = -1; if (p.status) p.status[seq] = s.misc[1]; }
+        return;
+    }
+    if (tid == 0 && p.status) p.status[seq] = 0;
+    for (int e = tid; e < NB * 4; e += C::NTHR) {
+        const int A = e >> 2, x = e & 3;
+        uint32_t bits = 0;
+#pragma unroll
+        for (int a = 0; a < Q; ++a) bits |= (uint32_t)rna4r_pair(s.code[A * Q + a], x) << a;
+        s.pm[e] = (uint8_t)bits;
+    }
+    // ---- tile-diagonal 0
+    for (int A = tid; A < NB; A += C::NTHR) diag_tile<Q, TABLE>(p, s, seq, A);
+    __syncthreads();
+
+    for (int D = 1; D < NB; ++D) {
+        const int NT = NB - D;
+        // ---- phase A: waves of diagonal D, early bulk of the strip-tiles that start on diagonal D+1
+        int wbase[C::G + 1];
+        wbase[0] = 0;
+#pragma unroll
+        for (int rho = 0; rho < C::G; ++rho) {
+            const int cnt = rho < NT ? (NT - rho + C::G - 1) / C::G : 0;
+            wbase[rho + 1] = wbase[rho] + (cnt + C::G - 1) / C::G;
+        }
+        const int ntw = wbase[C::G];
+        const int D0 = D + 1;
+        int Afirst, nE;
+        strips_of(NB, C::G, D0, Afirst, nE);
+        const int elen = D0 - 2 - C::G;                          // early groups A+G+1 .. A+D0-2 of a strip-tile
+        int P = 0;
+        if (nE > 0 && elen > 0) {
+            P = (C::NWARP - ntw) / nE;
+            P = P < 1 ? 1 : (P > 4 ? 4 : P);
+            if (P > elen) P = elen;
+            while (nE * P > C::PB_SLOTS) --P;
+        }
+        const int ntask = ntw + nE * P;
+        for (;;) {
+            int t = 0;
+            if (lane == 0) t = atomicAdd(&s.misc[0], 1);
+            t = __shfl_sync(0xffffffffu, t, 0);
+            if (t >= ntask) break;
+            if (t < ntw) {
+                int rho = 0;
+#pragma unroll
+                for (int r2 = 1; r2 < C::G; ++r2) if (t >= wbase[r2]) rho = r2;
+                wave_task<Q, TABLE>(p, s, seq, D, rho, t - wbase[rho], warp, lane);
+            } else {
+                const int e = t - ntw, ie = e / P, pe = e - ie * P;
+                const int A = Afirst + C::G * ie, GC = A + D0;
+                const int cx = min(GC * Q + lane, NB * Q - 1);
+                const int glo = A + C::G + 1 + (elen * pe) / P, ghi = A + C::G + (elen * (pe + 1)) / P;
+                uint32_t acc[Q];
+#pragma unroll
+                for (int a = 0; a < Q; ++a) acc[a] = 0;
+                strip_groups<Q>(s, A, cx, glo, ghi, acc);
+                s.part[e * 32 + lane] = pack_rows<Q>(acc);
+            }
+        }
+        __syncthreads();
+        // ---- phase B: the groups diagonal D completed, for the strip-tiles that start on diagonal D+1
+        if (tid == 0) s.misc[0] = 0;
+        for (int ie = warp; ie < nE; ie += C::NWARP) {
+            const int A = Afirst + C::G * ie, GC = A + D0;
+            const int cx = min(GC * Q + lane, NB * Q - 1);
+            uint32_t acc[Q];
+#pragma unroll
+            for (int a = 0; a < Q; ++a) acc[a] = 0;
+            for (int pe = 0; pe < P; ++pe) {
+                const uint32_t w = s.part[(ie * P + pe) * 32 + lane];
+#pragma unroll
+                for (int a = 0; a < Q; ++a) acc[a] = max(acc[a], (uint32_t)unpack_row<Q>(w, a));
+            }
+            strip_groups<Q>(s, A, cx, A + 1, min(A + C::G, GC - 1), acc);
+            if (GC - 1 > A + C::G) strip_groups<Q>(s, A, cx, GC - 1, GC - 1, acc);
+            s.val[A * 32 + lane] = pack_rows<Q>(acc);
+        }
+        __syncthreads();
+    }
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------------
+static inline size_t workspace_bytes(int count) { return 256 + 2 * align_up((size_t)(count > 0 ? count : 1) * 4, 256); }
+
+template <int Q>
+static int enqueue_q(rna4r_ctx *ctx, const uint8_t *seqs, const int64_t *offsets, const int32_t *lens_host, int count, int n_single,
+                     int32_t *scores, int32_t *status, void *table_out, int table_dtype, void *ws, cudaStream_t st)
+{
+    using C = Cfg<Q>;
+    Params p;
+    p.seqs = seqs; p.offsets = offsets; p.lens = nullptr; p.order = nullptr; p.n_single = n_single;
+    p.tbl = ctx->Rc; p.scores = scores; p.status = status; p.table_out = table_out; p.table_dtype = table_dtype;
+    int max_len = n_single;
+    if (offsets) {
+        // longest first: the hardware hands CTAs to SMs in index order, so this is the LPT rule (work ~ n^3).
+        // Counting sort by length into a context-owned host array (grown on demand, never per call).
+        if (count > ctx->order_cap) {
+            int32_t *nb = new (std::nothrow) int32_t[(size_t)count];
+            if (!nb) return RNA4R_ERR_CUDA;
+            delete[] ctx->order_host;
+            ctx->order_host = nb; ctx->order_cap = count;
+        }
+        max_len = 0;
+        for (int t = 0; t < count; ++t) if (lens_host[t] > max_len) max_len = lens_host[t];
+        {
+            int hist[2050] = {0};
+            if (max_len > 2048) return RNA4R_ERR_BAD_N;
+            for (int t = 0; t < count; ++t) ++hist[max_len - lens_host[t] + 1];
+            for (int b = 1; b <= max_len + 1; ++b) hist[b] += hist[b - 1];
+            for (int t = 0; t < count; ++t) ctx->order_host[hist[max_len - lens_host[t]]++] = t;
+        }
+        char *base = (char *)ws;
+        int32_t *lens_dev = (int32_t *)(base + 256);
+        int32_t *order_dev = (int32_t *)(base + 256 + align_up((size_t)count * 4, 256));
+        RNA4R_CUDA(ctx, cudaMemcpyAsync(lens_dev, lens_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
+        RNA4R_CUDA(ctx, cudaMemcpyAsync(order_dev, ctx->order_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
+        p.lens = lens_dev; p.order = order_dev;
+    }
+    if (max_len > max_n<Q>()) return RNA4R_ERR_BAD_N;
+    size_t smem = (size_t)C::FIXED_BYTES + make_layout<Q>(max_len).total;
+    if (smem < 49152) smem = 49152;
+    auto kern = table_out ? seq_kernel<Q, true> : seq_kernel<Q, false>;
+    RNA4R_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::MAX_SMEM));
+    if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
+    kern<<<count, C::NTHR, smem, st>>>(p);
+    if (ctx->timing) { RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev1, st)); ctx->timing_valid = 1; }
+    RNA4R_CUDA(ctx, cudaGetLastError());
+    ctx->last_launches = 1;
+    return RNA4R_OK;
+}
+
+}  // namespace smemseq
