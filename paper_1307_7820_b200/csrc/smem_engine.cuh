@@ -7,31 +7,34 @@
 // with h / v the q-1 informative difference bits of the row run / the column run (v_0 = 0).
 //
 // What is stored ("only the horizontal and vertical differences are stored", plus anchors, reading g21):
-//   W[g][r]  (r < gq)   row word of row r over group g, 32 bit:  h << 24 | M(r,gq)
-//   X[g][c]  (c >= gq)  column word of column c over group g, 16 bit:  v << (16-HB) | M(gq,c); expanded on load to
-//                       v << (24-HB) | M(gq,c), so that S = W + X has the table index h*2^HB + v at bit 24-HB and
-//                       the anchor sum in the low halfword: one lookup = add, LEA.HI, LDS.U8, VIADDMNMX.U16x2.
-// Nothing else of the table is kept: n^2/(2q) words of each kind (n = 700, q = 8: 122 KB + 61 KB).
+//   W[A][j][a]   row word of row Aq+a over group g = A+1+j, 32 bit:  h << 24 | M(r,gq)      (tile-row major)
+//   X[B][g][y]   column word of column Bq+y over group g <= B, 16 bit:  v << (16-HB) | M(gq,c); expanded on load to
+//                v << (24-HB) | M(gq,c), so that S = W + X has the table index h*2^HB + v at bit 24-HB and the
+//                anchor sum in the low halfword: one lookup = add, LEA.HI, LDS.U8, VIADDMNMX.U16x2.
+// Nothing else of the table is kept: n^2/(2q) words of each kind (n = 700, q = 8: 122 KB + 61 KB).  Both arrays are
+// laid out so that the groups a row block / a column meets one after another are a constant stride apart.
 //
 // Schedule.  q x q tiles (A,B); the tiles of one tile-diagonal D = B - A are independent.  For a tile
 // the groups strictly between A and B are complete for all its q^2 cells (Alg. 1 lines 15-19);
-// groups A and B are the paper's residual loops.  Per tile-diagonal step D, one CTA barrier apart:
-//   phase A   (i) waves: the closure of every tile of diagonal D, 4 tiles per warp (Q lanes each), and
-//             (ii) "early bulk" of diagonal D+1: for every strip-tile (tile-row A x 4 tile-columns = 32 columns) whose
-//             first tile lies on diagonal D+1, the complete groups that no tile of diagonal D feeds -- lanes <-> 32
-//             columns of ONE row, so the row word is warp-uniform and the table gather is conflict-free;
-//   phase B   the groups of those strip-tiles that diagonal D completed; the maxima are packed into one word per
-//             column (value of the bottom row + 3-bit offsets of the rows above: Lemma 1 bounds them by q-1).
-// The few groups a strip-tile cannot take for its 2nd..4th tile column ("fresh" groups, at most 3 per side) are
-// looked up inside the wave.
+// groups A and B are the paper's residual loops.  One CTA barrier per tile-diagonal step D; the
+// warps share, dealt round-robin,
+//   (i)  the waves: the closure of every tile of diagonal D, 4 tiles per warp (Q lanes each), and
+//   (ii) the bulk of diagonal D+1 and later: for every strip-tile (tile-row A x 4 tile-columns = 32 columns) whose
+//        first tile lies on diagonal D0 = D+1, the complete groups j = g-A-1 in [1, D0-3] that no tile of diagonal D
+//        feeds -- lanes <-> 32 columns of ONE row, so the row word is warp-uniform and the table gather is conflict-
+//        free.  The maxima are packed into one word per column (value of the bottom row + 3-bit offsets of the rows
+//        above: Lemma 1 bounds them by q-1) in a 5-slot ring per tile-row.
+// The groups a strip-tile cannot take yet ("fresh": j in [0,k] and [D0-2, D-2] for its k-th tile column, at most
+// 4 per side) are looked up inside the wave.
 //
 // Wave of tile (A,B), row-parallel: rows from the bottom up, the Q cells of a row at once.  With
-//   C'(a,y) = max{ bulk, b + M(r+1,c-1), head: max_{t in group A, t>r} M(r,t)+M(t,c) }   -- rows below only
+//   C'(a,y) = max{ bulk, fresh, b + M(r+1,c-1), head: max_{t in group A, t>r} M(r,t)+M(t,c) }   -- rows below only
 // the row is  V(a,y) = max_{y' <= y} C'(a,y') + Qd(y',y),  Qd = the diagonal tile (B,B): the in-row dependency
 // V(a,y) >= V(a,y') + Qd(y',y) collapses because Qd is superadditive (M(i,k) >= M(i,j) + M(j,k)).  The head is one
 // masked lookup with the running column word; the tail is a max-plus over the row's packed C' values
 // (4 DPX VIADDMNMX.S16x2).  No skewed wavefront: 8 dependent steps per tile, every lane busy in every step.
 #pragma once
+#include <new>
 #include "common.cuh"
 
 namespace smemseq {
@@ -52,10 +55,10 @@ struct Cfg {
     static constexpr int NWARP = 24;
     static constexpr int NTHR = NWARP * 32;
     static constexpr int NP = (Q + 1) / 2;           // packed value pairs of a tile row
-    static constexpr int NF = G - 1;                 // fresh groups per side
-    static constexpr int PB_SLOTS = 32;              // partial-maximum rows between phase A and phase B
     static constexpr int VBITS = 11;                 // value bits of a packed bulk word (D <= 2047)
-    static constexpr int SCR_BYTES = NWARP * 2 * G * 16;   // per-warp row scratch: [2][G] x 8 halfwords
+    static constexpr int VPITCH = 40;                // words per tile-row of the bulk ring: 5 tile-column slots x 8
+    static constexpr int SCR_WARP_HW = 2 * G * 8 + 8 * 2 + 8;    // per-warp scratch in halfwords: row buffers [2][G][8], two dummy store targets
+    static constexpr int SCR_BYTES = NWARP * SCR_WARP_HW * 2;
     static constexpr int FIXED_BYTES = TBL_AREA + SCR_BYTES + 64;
     static constexpr int MAX_SMEM = 232448;          // 227 KB
 };
@@ -63,7 +66,7 @@ struct Cfg {
 // byte offsets of one sequence's state, relative to the start of the pool
 struct Layout {
     int NB;
-    uint32_t W, X, val, wdh, dq, pm, rl, code, part, total;
+    uint32_t W, X, val, wdh, dq, pm, rl, code, total;
 };
 
 template <int Q>
@@ -76,13 +79,12 @@ __host__ __device__ inline Layout make_layout(int n)
     auto take = [&](uint32_t bytes) { const uint32_t o = off; off += (bytes + 15u) & ~15u; return o; };
     L.W = take(4u * Q * NB * (NB - 1) / 2);
     L.X = take(2u * Q * NB * (NB + 1) / 2);
-    L.val = take(4u * 32u * NB);
+    L.val = take(4u * Cfg<Q>::VPITCH * (NB + 1));
     L.wdh = take(4u * Q * NB);
     L.dq = take(8u * Q * NB);
     L.pm = take(4u * NB);
     L.rl = take(2u * Q * NB);
     L.code = take(Q * NB + 16u);
-    L.part = take(4u * 32u * Cfg<Q>::PB_SLOTS);
     L.total = off;
     return L;
 }
@@ -113,13 +115,15 @@ struct Params {
     int32_t *status;          // NULL or [count]
     void *table_out;          // NULL, or n*n elements (single sequence only)
     int table_dtype;
+    unsigned long long *trace;   // NULL, or [trace_seqs][8] clock64 sums of warp 0 (rna4r_set_trace): total, setup + diagonal
+    int trace_seqs;              // tiles, waves + bulk, merge phases, wave tasks, #wave tasks, bulk tasks, n
 };
 
 template <int Q>
 struct Sm {
     uint32_t tbl_sa;          // shared-space address of the table
     uint16_t *scr;            // per-warp row scratch
-    int *misc;                // [0] task counter, [1] invalid flag
+    int *misc;                // [1] invalid flag
     uint32_t *W;
     uint16_t *X;
     uint32_t *val;
@@ -128,7 +132,6 @@ struct Sm {
     uint8_t *pm;
     int16_t *rl;
     int8_t *code;
-    uint32_t *part;
     int n, NB;
 };
 
@@ -147,8 +150,24 @@ __device__ __forceinline__ uint32_t lookup_max(uint32_t tbl_sa, uint32_t S, uint
 template <int Q>
 __device__ __forceinline__ uint32_t expand_x(uint32_t x16) { return x16 + (x16 >> Cfg<Q>::XAB) * Cfg<Q>::XMUL; }
 
-template <int Q> __device__ __forceinline__ int off_w(int g) { return Q * (g * (g - 1) / 2); }                 // words
-template <int Q> __device__ __forceinline__ int off_x(int NB, int g) { return Q * (g * NB - g * (g - 1) / 2); } // halfwords
+template <int Q> __device__ __forceinline__ int off_w(int NB, int A) { return Q * (A * (NB - 1) - A * (A - 1) / 2); }   // words
+template <int Q> __device__ __forceinline__ int off_x(int B) { return Q * (B * (B + 1) / 2); }                          // halfwords
+
+// the Q row words of tile-row A over one group (warp- or tile-uniform address: broadcast loads)
+template <int Q>
+__device__ __forceinline__ void load_rows(const uint32_t *w, uint32_t (&wr)[Q])
+{
+    if constexpr (Q % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < Q / 4; ++i) {
+            const uint4 t = reinterpret_cast<const uint4 *>(w)[i];
+            wr[4 * i] = t.x; wr[4 * i + 1] = t.y; wr[4 * i + 2] = t.z; wr[4 * i + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int a = 0; a < Q; ++a) wr[a] = w[a];
+    }
+}
 
 // step a8 for the test / inspection path: out[(i-1)*n + (j-1)] = D(i,j) = M(i-1, j)
 template <bool TABLE>
@@ -159,35 +178,6 @@ __device__ __forceinline__ void store_cell(const Params &p, int n, int r, int c,
             if (p.table_dtype == RNA4R_TABLE_INT16) reinterpret_cast<int16_t *>(p.table_out)[(size_t)r * n + c - 1] = (int16_t)v;
             else reinterpret_cast<int32_t *>(p.table_out)[(size_t)r * n + c - 1] = v;
         }
-    }
-}
-
-// ---- bulk (step a4): rows of tile-row A x the 32 columns of a strip, groups glo..ghi --------------------------------
-// lane <-> column cx, a thread owns the Q rows; the row words are warp-uniform (broadcast loads), so all 32 gathers
-// of a lookup fall in one table row: conflict-free.
-template <int Q>
-__device__ __forceinline__ void strip_groups(const Sm<Q> &s, int A, int cx, int glo, int ghi, uint32_t (&acc)[Q])
-{
-    const uint32_t *w = s.W + off_w<Q>(glo) + A * Q;
-    const uint16_t *x = s.X + off_x<Q>(s.NB, glo) - glo * Q + cx;
-#pragma unroll 2
-    for (int g = glo; g <= ghi; ++g) {
-        const uint32_t X32 = expand_x<Q>(*x);
-        uint32_t wr[Q];
-        if constexpr (Q % 4 == 0) {
-#pragma unroll
-            for (int i = 0; i < Q / 4; ++i) {
-                const uint4 t = reinterpret_cast<const uint4 *>(w)[i];
-                wr[4 * i] = t.x; wr[4 * i + 1] = t.y; wr[4 * i + 2] = t.z; wr[4 * i + 3] = t.w;
-            }
-        } else {
-#pragma unroll
-            for (int a = 0; a < Q; ++a) wr[a] = w[a];
-        }
-#pragma unroll
-        for (int a = 0; a < Q; ++a) acc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, acc[a]);
-        w += Q * g;
-        x += Q * (s.NB - g - 1);
     }
 }
 
@@ -209,6 +199,44 @@ __device__ __forceinline__ int unpack_row(uint32_t w, int a)
     const int base = (int)(w & ((1u << Cfg<Q>::VBITS) - 1u));
     return a == Q - 1 ? base : base + (int)((w >> (Cfg<Q>::VBITS + 3 * a)) & 7u);
 }
+
+// ---- bulk (step a4): rows of tile-row A x the 32 columns of the strip that starts at tile column GC -----------------
+// Groups j = g-A-1 in [jlo, jhi] (1 <= jlo).  lane <-> column, a thread owns the Q rows; the row words are warp-uniform
+// (broadcast loads), so all 32 gathers of a lookup fall in one table row: conflict-free.  Group j of the strip's k-th
+// tile column comes from tile (A+1+j, GC+k), which is finished only if j > k: the lanes of later tile columns sit
+// out j = 1..3 (their share is looked up in the wave).
+template <int Q>
+__device__ __forceinline__ void strip_bulk(const Sm<Q> &s, int A, int GC, int jlo, int jhi, int lane, uint32_t (&acc)[Q])
+{
+    using C = Cfg<Q>;
+    const int l2 = lane < C::SW ? lane : C::SW - 1;
+    const int kq = l2 / Q, y = l2 - kq * Q;
+    const int Bc = min(GC + kq, s.NB - 1);
+    const uint32_t *w = s.W + off_w<Q>(s.NB, A) + jlo * Q;
+    const uint16_t *x = s.X + off_x<Q>(Bc) + (A + 1 + jlo) * Q + y;
+    int j = jlo;
+    for (; j <= jhi && j <= C::G - 1; ++j) {
+        const uint32_t X32 = (kq < j) ? expand_x<Q>(*x) : 0u;             // X = 0: a valid lower bound, nothing read
+        uint32_t wr[Q];
+        load_rows<Q>(w, wr);
+#pragma unroll
+        for (int a = 0; a < Q; ++a) acc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, acc[a]);
+        w += Q; x += Q;
+    }
+#pragma unroll 4
+    for (; j <= jhi; ++j) {
+        const uint32_t X32 = expand_x<Q>(*x);
+        uint32_t wr[Q];
+        load_rows<Q>(w, wr);
+#pragma unroll
+        for (int a = 0; a < Q; ++a) acc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, acc[a]);
+        w += Q; x += Q;
+    }
+}
+
+// ring slot of (tile-row A, tile column Bc, column y) in the packed bulk maxima
+template <int Q>
+__device__ __forceinline__ int val_index(int A, int Bc, int y) { return A * Cfg<Q>::VPITCH + (Bc % 5) * 8 + y; }
 
 // ---- diagonal tile (A,A): plain eq. (1) on Q x Q cells, one thread --------------------------------------------------
 template <int Q, bool TABLE>
@@ -235,7 +263,7 @@ __device__ void diag_tile(const Params &p, const Sm<Q> &s, int seq, int A)
             m[a][y] = best;
         }
     }
-    uint16_t *xo = s.X + off_x<Q>(s.NB, A);
+    uint16_t *xo = s.X + off_x<Q>(A) + A * Q;
 #pragma unroll
     for (int y = 0; y < Q; ++y) {
         uint32_t vb = 0;
@@ -266,48 +294,51 @@ __device__ void diag_tile(const Params &p, const Sm<Q> &s, int seq, int A)
     }
 }
 
-// ---- wave: closure of up to G tiles of tile-diagonal D, residue class rho = A mod G, task jt ------------------------
+// ---- wave: closure of up to G tiles of tile-diagonal D --------------------------------------------------------------
+// Task t = 4*jt + rho takes the tiles A = rho + 16*jt + 4*i, i = 0..3 (lane group i): they share k = (A + D) mod 4
+// and D0 = D - k (the diagonal their strip-tile starts on), so every loop bound below is warp-uniform.
 template <int Q, bool TABLE>
-__device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int seq, int D, int rho, int jt, int warp, int lane)
+__device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int seq, int D, int t, int warp, int lane)
 {
     using C = Cfg<Q>;
     constexpr uint32_t FULL = 0xffffffffu;
     const int NB = s.NB, NT = NB - D;
+    const int A0 = (t & 3) + 16 * (t >> 2);
+    if (A0 >= NT) return;
     const bool lane_ok = lane < C::SW;
     const int i = lane_ok ? lane / Q : C::G - 1;
     const int y = lane_ok ? lane - i * Q : Q - 1;
-    const int cnt = (NT - rho + C::G - 1) / C::G;              // tiles of this residue class on the diagonal
-    int j = jt * C::G + i;
-    const bool own = lane_ok && j < cnt;
-    if (j >= cnt) j = jt * C::G;                               // shadow of the first tile: computes, stores nothing
-    const int A = rho + C::G * j, B = A + D;
-    const int k = B % C::G, GC = B - k, D0 = D - k;            // k, D0: the same for every tile of the task
+    int A = A0 + C::G * i;
+    const bool own = lane_ok && A < NT;
+    if (A >= NT) A = A0;                                       // shadow of the first tile: computes, stores nothing
+    const int B = A + D;
+    const int k = B & (C::G - 1), D0 = D - k;
     const int r0 = A * Q, c = B * Q + y;
+    const uint16_t *xcol = s.X + off_x<Q>(B) + y;              // xcol[g*Q] = column word of (group g, my column)
+    const uint32_t *wrow = s.W + off_w<Q>(NB, A);              // wrow[j*Q + a] = row word of (row r0+a, group A+1+j)
 
-    // bulk maxima of the strip-tile (phase B of step D0 - 1); none before the strip-tile's first diagonal is 2
-    uint32_t vw = 0;
-    if (D0 >= 2) vw = s.val[A * 32 + k * Q + y];
-    // fresh groups: head side A+1 .. A+nfh (column words of the tiles below), tail side GC .. GC+nft-1 (row words of
-    // the tiles to the left inside the strip).  Without bulk (D0 < 2) the D-1 complete groups are all fresh.
-    const int nfh = (D0 >= 2) ? k : D - 1;
-    const int nft = (D0 >= 2) ? k : 0;
-    uint32_t Xf[2 * C::NF];
-    const uint32_t *Wf[2 * C::NF];
+    // ---- fresh groups (a4): j in [0, min(k, D-2)] (column words of the tiles just below) and from max(D0-2, k+1) to
+    // D-2 (row words of the tiles to the left inside the strip); without bulk (D0 < 4) that is every complete group
+    uint32_t facc[Q];
 #pragma unroll
-    for (int t = 0; t < C::NF; ++t) {
-        Xf[t] = 0; Wf[t] = s.W;
-        if (t < nfh) {
-            const int g = A + 1 + t;
-            Xf[t] = expand_x<Q>(s.X[off_x<Q>(NB, g) + c - g * Q]);
-            Wf[t] = s.W + off_w<Q>(g) + r0;
-        }
-        Xf[C::NF + t] = 0; Wf[C::NF + t] = s.W;
-        if (t < nft) {
-            const int g = GC + t;
-            Xf[C::NF + t] = expand_x<Q>(s.X[off_x<Q>(NB, g) + c - g * Q]);
-            Wf[C::NF + t] = s.W + off_w<Q>(g) + r0;
+    for (int a = 0; a < Q; ++a) facc[a] = 0;
+    {
+        const int j1 = min(k, D - 2), j2 = max(D0 - 2, k + 1);
+        const int nf = (j1 + 1) + max(D - 1 - j2, 0);
+        int j = 0;
+#pragma unroll 1
+        for (int f = 0; f < nf; ++f) {
+            const uint32_t X32 = expand_x<Q>(xcol[(A + 1 + j) * Q]);
+            uint32_t wr[Q];
+            load_rows<Q>(wrow + j * Q, wr);
+#pragma unroll
+            for (int a = 0; a < Q; ++a) facc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, facc[a]);
+            j = (j == j1) ? j2 : j + 1;
         }
     }
+    // bulk maxima of the strip-tile, written during step D0 - 1 (none if the strip-tile starts before diagonal 4)
+    uint32_t vw = 0;
+    if (D0 >= 4) vw = s.val[val_index<Q>(A, B, y)];
     // diagonal tile (B,B) for the tail: packed pairs (Qd(2j,y), Qd(2j+1,y)); y' > y is "minus infinity"
     int Qp[C::NP];
     {
@@ -329,33 +360,31 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
     }
     // bottom edge M((A+1)q, c): anchor of the column word of group A+1; left column M(r0+1+y, Bq-1) for lane 0's
     // pair term: the last value tile (A,B-1) left in its rows, and for the row below the tile an anchor again
-    const uint16_t *xbelow = s.X + off_x<Q>(NB, A + 1) - (A + 1) * Q;
-    int vprev = (int)(xbelow[c] & C::XAMASK);
+    int vprev = (int)(xcol[(A + 1) * Q] & C::XAMASK);
     int Lc;
     if (y < Q - 1) Lc = s.rl[r0 + 1 + y];
-    else Lc = (D >= 2) ? (int)(xbelow[B * Q - 1] & C::XAMASK) : 0;
+    else Lc = (D >= 2) ? (int)(s.X[off_x<Q>(B - 1) + (A + 1) * Q + Q - 1] & C::XAMASK) : 0;
     const uint32_t *wh = s.wdh + r0;
-    uint16_t *scr = s.scr + (size_t)warp * (2 * C::G * 8);
-    uint32_t *wout = s.W + off_w<Q>(B) + r0;
-    uint32_t xbits = 0;
+    uint16_t *scr = s.scr + (size_t)warp * C::SCR_WARP_HW;
+    // lanes that own no output store to a per-warp dummy word instead of predicating every store
+    uint32_t *wout = (own && y == 0) ? const_cast<uint32_t *>(wrow) + (D - 1) * Q : reinterpret_cast<uint32_t *>(scr + 2 * C::G * 8);
+    int16_t *rlo = (own && y == Q - 1) ? s.rl + r0 : reinterpret_cast<int16_t *>(scr + 2 * C::G * 8 + 16);
+    const int bsh = i * Q + 1;
+    uint16_t *rowbase = scr + i * 8;
     uint32_t Xp = (uint32_t)vprev;
     int vl = __shfl_sync(FULL, vprev, lane - 1);                  // M(r+1, c-1) for the bottom row
     int v = 0;
 #pragma unroll
     for (int a = Q - 1; a >= 0; --a) {
-        // ---- candidates from the rows below: bulk, pair term (a3), head residual (a5), fresh groups (a4)
+        // ---- candidates from the rows below: bulk, fresh, pair term (a3), head residual (a5)
         const int lca = __shfl_sync(FULL, Lc, i * Q + a);
         const int vd = (y == 0) ? lca : vl;
         int cand = unpack_row<Q>(vw, a);
         cand = max(cand, vd + (int)((pm >> a) & 1u));
         uint32_t best = lookup_max<Q>(s.tbl_sa, wh[a] + Xp, (uint32_t)cand);
-#pragma unroll
-        for (int t = 0; t < 2 * C::NF; ++t) {
-            const bool on = (t < C::NF) ? (t < nfh) : (t - C::NF < nft);          // warp-uniform
-            if (on) best = lookup_max<Q>(s.tbl_sa, Wf[t][a] + Xf[t], best);
-        }
+        best = __vmaxu2(best, facc[a]);
         // ---- tail: V(a,y) = max_{y' <= y} C'(a,y') + Qd(y',y)
-        uint16_t *row = scr + ((a & 1) * C::G + i) * 8;
+        uint16_t *row = rowbase + (a & 1) * (C::G * 8);
         if (lane_ok) row[y] = (uint16_t)(best & 0xffffu);
         __syncwarp();
         int m2 = (int)0x80008000u;
@@ -374,30 +403,25 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
         // ---- step a6: row word of row r over group B (ballot of the horizontal differences), column word bit
         vl = __shfl_sync(FULL, v, lane - 1);
         const uint32_t bal = __ballot_sync(FULL, y > 0 && v != vl);
-        if (own && y == 0) wout[a] = (((bal >> (i * Q + 1)) & C::HMASK) << 24) | (uint32_t)v;
-        if (own && y == Q - 1) s.rl[r0 + a] = (int16_t)v;
-        if (a < Q - 1) xbits |= (uint32_t)(v - vprev) << (C::ISH + a);
-        Xp = xbits | (uint32_t)v;
+        wout[a] = (((bal >> bsh) & C::HMASK) << 24) | (uint32_t)v;
+        rlo[a] = (int16_t)v;
+        // column word: the anchor moves up to row a, the difference to the row below enters at index bit a
+        if (a == Q - 1) Xp = (uint32_t)v;
+        else Xp += (uint32_t)(v - vprev) * (1u + (1u << (C::ISH + a)));
         vprev = v;
         if (own) store_cell<TABLE>(p, s.n, r0 + a, c, v);
     }
     if (own) {
-        s.X[off_x<Q>(NB, A) + c - A * Q] = (uint16_t)(((xbits >> C::ISH) << C::XAB) | (uint32_t)v);
+        const_cast<uint16_t *>(xcol)[A * Q] = (uint16_t)(((Xp >> C::ISH) << C::XAB) | (Xp & 0xffffu));
         if (A == 0 && c == s.n) p.scores[seq] = v;                // M(0,n) = D(1,n)
     }
-}
-
-// strip-tiles whose first tile lies on diagonal D0: A = Afirst + G*i, i < nE
-__device__ __forceinline__ void strips_of(int NB, int G, int D0, int &Afirst, int &nE)
-{
-    Afirst = (G - D0 % G) % G;
-    nE = (D0 < NB && NB - 1 - D0 >= Afirst) ? (NB - 1 - D0 - Afirst) / G + 1 : 0;
 }
 
 template <int Q, bool TABLE>
 __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
 {
     using C = Cfg<Q>;
+    static_assert(C::G == 4, "task numbering assumes 4 tiles per warp");
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int seq = p.order ? p.order[blockIdx.x] : (int)blockIdx.x;
@@ -411,14 +435,18 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         s.misc = (int *)b; b += 64;
         s.W = (uint32_t *)(b + L.W); s.X = (uint16_t *)(b + L.X); s.val = (uint32_t *)(b + L.val);
         s.wdh = (uint32_t *)(b + L.wdh); s.dq = b + L.dq; s.pm = b + L.pm; s.rl = (int16_t *)(b + L.rl);
-        s.code = (int8_t *)(b + L.code); s.part = (uint32_t *)(b + L.part);
+        s.code = (int8_t *)(b + L.code);
         s.n = n; s.NB = L.NB;
         uint32_t dyn;
         asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
         if ((uint32_t)C::FIXED_BYTES + L.total > dyn) __trap();       // the host routes longer sequences elsewhere: fail loudly
     }
     const int NB = s.NB;
-    // ---- setup: table, codes (step a1), zeroed column words (an unwritten word is a valid lower bound)
+    unsigned long long *tr = (p.trace && seq < p.trace_seqs) ? p.trace + (size_t)seq * RNA4R_TRACE_WORDS : nullptr;
+    long long t_start = 0, t_a = 0, t_b = 0, t_wave = 0, t_early = 0, t_setup = 0;
+    int n_wave = 0;
+    if (tr) t_start = clock64();
+    // ---- setup: table, codes (step a1)
     {
         const uint32_t *src = reinterpret_cast<const uint32_t *>(p.tbl);
         uint32_t *dst = reinterpret_cast<uint32_t *>(smem_raw);
@@ -437,9 +465,6 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
             s.code[x] = (int8_t)cde;
         }
         if (bad) atomicOr(&s.misc[1], bad);
-        uint4 *xz = reinterpret_cast<uint4 *>(s.X);
-        const int nx = (int)((L.val - L.X) / 16);
-        for (int e = tid; e < nx; e += C::NTHR) xz[e] = make_uint4(0, 0, 0, 0);
     }
     __syncthreads();
     if (s.misc[1]) {                                   // reading g4: not a base -> score -1, status word
@@ -457,71 +482,71 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
     // ---- tile-diagonal 0
     for (int A = tid; A < NB; A += C::NTHR) diag_tile<Q, TABLE>(p, s, seq, A);
     __syncthreads();
+    if (tr) t_setup = clock64() - t_start;
 
     for (int D = 1; D < NB; ++D) {
+        long long ta0 = 0, tb0 = 0;
+        if (tr) ta0 = clock64();
         const int NT = NB - D;
-        // ---- phase A: waves of diagonal D, early bulk of the strip-tiles that start on diagonal D+1
-        int wbase[C::G + 1];
-        wbase[0] = 0;
-#pragma unroll
-        for (int rho = 0; rho < C::G; ++rho) {
-            const int cnt = rho < NT ? (NT - rho + C::G - 1) / C::G : 0;
-            wbase[rho + 1] = wbase[rho] + (cnt + C::G - 1) / C::G;
-        }
-        const int ntw = wbase[C::G];
+        // Tasks of the step, dealt round-robin to the warps, waves first.  Bulk tasks: the strip-tiles (A, GC = A + D0)
+        // that start on diagonal D0 = D+1 >= 4, groups j in [1, D0-3]; when warps would otherwise idle the range is
+        // split in 2 or 4 parts, which leave their maxima in dead rows of the ring (tile-rows >= NT have no tile left)
+        // and are merged after an extra barrier.
+        const int ntw = 4 * ((NT + 15) >> 4);
         const int D0 = D + 1;
-        int Afirst, nE;
-        strips_of(NB, C::G, D0, Afirst, nE);
-        const int elen = D0 - 2 - C::G;                          // early groups A+G+1 .. A+D0-2 of a strip-tile
-        int P = 0;
-        if (nE > 0 && elen > 0) {
-            P = (C::NWARP - ntw) / nE;
-            P = P < 1 ? 1 : (P > 4 ? 4 : P);
-            if (P > elen) P = elen;
-            while (nE * P > C::PB_SLOTS) --P;
+        const int Afirst = (4 - (D0 & 3)) & 3;
+        const int nE = (D0 >= 4 && D0 < NB && NB - 1 - D0 >= Afirst) ? ((NB - 1 - D0 - Afirst) >> 2) + 1 : 0;
+        const int elen = D0 - 3;
+        int lp = 0;
+        if (nE > 0) {
+            const int wfree = C::NWARP - (NT + 3) / 4;
+            const int rows = (D * C::VPITCH) / 32;               // part slots (32 words each) the dead rows hold
+            lp = (elen >= 72 && 4 * nE <= wfree && 4 * nE <= rows) ? 2 : (elen >= 40 && 2 * nE <= wfree && 2 * nE <= rows) ? 1 : 0;
         }
-        const int ntask = ntw + nE * P;
-        for (;;) {
-            int t = 0;
-            if (lane == 0) t = atomicAdd(&s.misc[0], 1);
-            t = __shfl_sync(0xffffffffu, t, 0);
-            if (t >= ntask) break;
+        uint32_t *part = s.val + NT * C::VPITCH;
+        const int ntask = ntw + (nE << lp);
+        for (int t = warp; t < ntask; t += C::NWARP) {
+            long long tt0 = 0;
+            if (tr) tt0 = clock64();
             if (t < ntw) {
-                int rho = 0;
-#pragma unroll
-                for (int r2 = 1; r2 < C::G; ++r2) if (t >= wbase[r2]) rho = r2;
-                wave_task<Q, TABLE>(p, s, seq, D, rho, t - wbase[rho], warp, lane);
+                wave_task<Q, TABLE>(p, s, seq, D, t, warp, lane);
+                if (tr) { t_wave += clock64() - tt0; ++n_wave; }
             } else {
-                const int e = t - ntw, ie = e / P, pe = e - ie * P;
+                const int e = t - ntw, ie = e >> lp, pe = e & ((1 << lp) - 1);
                 const int A = Afirst + C::G * ie, GC = A + D0;
-                const int cx = min(GC * Q + lane, NB * Q - 1);
-                const int glo = A + C::G + 1 + (elen * pe) / P, ghi = A + C::G + (elen * (pe + 1)) / P;
                 uint32_t acc[Q];
 #pragma unroll
                 for (int a = 0; a < Q; ++a) acc[a] = 0;
-                strip_groups<Q>(s, A, cx, glo, ghi, acc);
-                s.part[e * 32 + lane] = pack_rows<Q>(acc);
+                strip_bulk<Q>(s, A, GC, 1 + ((elen * pe) >> lp), (elen * (pe + 1)) >> lp, lane, acc);
+                const uint32_t w = pack_rows<Q>(acc);
+                if (lp > 0) part[e * 32 + lane] = w;
+                else if (lane < C::SW && GC + lane / Q < NB) s.val[val_index<Q>(A, GC + lane / Q, lane % Q)] = w;
+                if (tr) t_early += clock64() - tt0;
             }
         }
         __syncthreads();
-        // ---- phase B: the groups diagonal D completed, for the strip-tiles that start on diagonal D+1
-        if (tid == 0) s.misc[0] = 0;
-        for (int ie = warp; ie < nE; ie += C::NWARP) {
-            const int A = Afirst + C::G * ie, GC = A + D0;
-            const int cx = min(GC * Q + lane, NB * Q - 1);
-            uint32_t acc[Q];
+        if (tr) { tb0 = clock64(); t_a += tb0 - ta0; }
+        if (lp > 0) {
+            for (int ie = warp; ie < nE; ie += C::NWARP) {
+                const int A = Afirst + C::G * ie, GC = A + D0;
+                uint32_t acc[Q];
 #pragma unroll
-            for (int a = 0; a < Q; ++a) acc[a] = 0;
-            for (int pe = 0; pe < P; ++pe) {
-                const uint32_t w = s.part[(ie * P + pe) * 32 + lane];
+                for (int a = 0; a < Q; ++a) acc[a] = 0;
+                for (int pe = 0; pe < (1 << lp); ++pe) {
+                    const uint32_t w = part[((ie << lp) + pe) * 32 + lane];
 #pragma unroll
-                for (int a = 0; a < Q; ++a) acc[a] = max(acc[a], (uint32_t)unpack_row<Q>(w, a));
+                    for (int a = 0; a < Q; ++a) acc[a] = max(acc[a], (uint32_t)unpack_row<Q>(w, a));
+                }
+                if (lane < C::SW && GC + lane / Q < NB) s.val[val_index<Q>(A, GC + lane / Q, lane % Q)] = pack_rows<Q>(acc);
             }
-            strip_groups<Q>(s, A, cx, A + 1, min(A + C::G, GC - 1), acc);
-            if (GC - 1 > A + C::G) strip_groups<Q>(s, A, cx, GC - 1, GC - 1, acc);
-            s.val[A * 32 + lane] = pack_rows<Q>(acc);
+            __syncthreads();
         }
-        __syncthreads();
+        if (tr) t_b += clock64() - tb0;
+    }
+    if (tr && tid == 0) {
+        tr[0] = (unsigned long long)(clock64() - t_start); tr[1] = (unsigned long long)t_setup; tr[2] = (unsigned long long)t_a;
+        tr[3] = (unsigned long long)t_b; tr[4] = (unsigned long long)t_wave; tr[5] = (unsigned long long)n_wave;
+        tr[6] = (unsigned long long)t_early; tr[7] = (unsigned long long)n;
     }
 }
 
@@ -536,6 +561,7 @@ static int enqueue_q(rna4r_ctx *ctx, const uint8_t *seqs, const int64_t *offsets
     Params p;
     p.seqs = seqs; p.offsets = offsets; p.lens = nullptr; p.order = nullptr; p.n_single = n_single;
     p.tbl = ctx->Rc; p.scores = scores; p.status = status; p.table_out = table_out; p.table_dtype = table_dtype;
+    p.trace = ctx->trace; p.trace_seqs = ctx->trace_tiles;
     int max_len = n_single;
     if (offsets) {
         // longest first: the hardware hands CTAs to SMs in index order, so this is the LPT rule (work ~ n^3).
