@@ -52,7 +52,10 @@ struct Cfg {
     static constexpr uint32_t HMASK = (1u << HB) - 1u;
     static constexpr int TBL_BYTES = 1 << (2 * HB);
     static constexpr int TBL_AREA = TBL_BYTES < 256 ? 256 : TBL_BYTES;
-    static constexpr int NWARP = 24;
+#ifndef RNA4R_SMEM_NWARP
+#define RNA4R_SMEM_NWARP 24
+#endif
+    static constexpr int NWARP = RNA4R_SMEM_NWARP;   // 80 registers per thread x 768 threads: the register file of one SM
     static constexpr int NTHR = NWARP * 32;
     static constexpr int NP = (Q + 1) / 2;           // packed value pairs of a tile row
     static constexpr int VBITS = 11;                 // value bits of a packed bulk word (D <= 2047)
@@ -66,7 +69,7 @@ struct Cfg {
 // byte offsets of one sequence's state, relative to the start of the pool
 struct Layout {
     int NB;
-    uint32_t W, X, val, wdh, dq, pm, rl, code, total;
+    uint32_t W, X, val, wdh, dq, pm, rl, code, plan, total;
 };
 
 template <int Q>
@@ -85,6 +88,7 @@ __host__ __device__ inline Layout make_layout(int n)
     L.pm = take(4u * NB);
     L.rl = take(2u * Q * NB);
     L.code = take(Q * NB + 16u);
+    L.plan = take(4u * NB);
     L.total = off;
     return L;
 }
@@ -132,6 +136,7 @@ struct Sm {
     uint8_t *pm;
     int16_t *rl;
     int8_t *code;
+    uint32_t *plan;           // [NB] step_plan of every tile-diagonal
     int n, NB;
 };
 
@@ -417,6 +422,29 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
     }
 }
 
+// Plan of tile-diagonal step D: ntw wave tasks | nE bulk tasks << 8 | first tile-row of a bulk task << 16 | log2(parts)
+// << 20.  Bulk tasks: the strip-tiles (A, GC = A + D0) that start on diagonal D0 = D+1 >= 4, groups j in [1, D0-3]; when
+// warps would otherwise idle behind one long bulk task the range is split in 2 or 4 parts, which leave their maxima in
+// dead rows of the ring (tile-rows >= NB-D have no tile left) and are merged after an extra barrier.
+template <int Q>
+__device__ __forceinline__ uint32_t step_plan(int NB, int D)
+{
+    using C = Cfg<Q>;
+    const int NT = NB - D;
+    const int ntw = 4 * ((NT + 15) >> 4);
+    const int D0 = D + 1;
+    const int Afirst = (4 - (D0 & 3)) & 3;
+    const int nE = (D0 >= 4 && D0 < NB && NB - 1 - D0 >= Afirst) ? ((NB - 1 - D0 - Afirst) >> 2) + 1 : 0;
+    const int elen = D0 - 3;
+    int lp = 0;
+    if (nE > 0) {
+        const int wfree = C::NWARP - (NT + 3) / 4;
+        const int rows = (D * C::VPITCH) / 32;               // part slots (32 words each) the dead rows hold
+        lp = (elen >= 72 && 4 * nE <= wfree && 4 * nE <= rows) ? 2 : (elen >= 40 && 2 * nE <= wfree && 2 * nE <= rows) ? 1 : 0;
+    }
+    return (uint32_t)ntw | ((uint32_t)nE << 8) | ((uint32_t)Afirst << 16) | ((uint32_t)lp << 20);
+}
+
 template <int Q, bool TABLE>
 __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
 {
@@ -435,7 +463,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         s.misc = (int *)b; b += 64;
         s.W = (uint32_t *)(b + L.W); s.X = (uint16_t *)(b + L.X); s.val = (uint32_t *)(b + L.val);
         s.wdh = (uint32_t *)(b + L.wdh); s.dq = b + L.dq; s.pm = b + L.pm; s.rl = (int16_t *)(b + L.rl);
-        s.code = (int8_t *)(b + L.code);
+        s.code = (int8_t *)(b + L.code); s.plan = (uint32_t *)(b + L.plan);
         s.n = n; s.NB = L.NB;
         uint32_t dyn;
         asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
@@ -479,6 +507,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         for (int a = 0; a < Q; ++a) bits |= (uint32_t)rna4r_pair(s.code[A * Q + a], x) << a;
         s.pm[e] = (uint8_t)bits;
     }
+    for (int D = tid; D < NB; D += C::NTHR) s.plan[D] = step_plan<Q>(NB, D);
     // ---- tile-diagonal 0
     for (int A = tid; A < NB; A += C::NTHR) diag_tile<Q, TABLE>(p, s, seq, A);
     __syncthreads();
@@ -488,21 +517,10 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         long long ta0 = 0, tb0 = 0;
         if (tr) ta0 = clock64();
         const int NT = NB - D;
-        // Tasks of the step, dealt round-robin to the warps, waves first.  Bulk tasks: the strip-tiles (A, GC = A + D0)
-        // that start on diagonal D0 = D+1 >= 4, groups j in [1, D0-3]; when warps would otherwise idle the range is
-        // split in 2 or 4 parts, which leave their maxima in dead rows of the ring (tile-rows >= NT have no tile left)
-        // and are merged after an extra barrier.
-        const int ntw = 4 * ((NT + 15) >> 4);
-        const int D0 = D + 1;
-        const int Afirst = (4 - (D0 & 3)) & 3;
-        const int nE = (D0 >= 4 && D0 < NB && NB - 1 - D0 >= Afirst) ? ((NB - 1 - D0 - Afirst) >> 2) + 1 : 0;
-        const int elen = D0 - 3;
-        int lp = 0;
-        if (nE > 0) {
-            const int wfree = C::NWARP - (NT + 3) / 4;
-            const int rows = (D * C::VPITCH) / 32;               // part slots (32 words each) the dead rows hold
-            lp = (elen >= 72 && 4 * nE <= wfree && 4 * nE <= rows) ? 2 : (elen >= 40 && 2 * nE <= wfree && 2 * nE <= rows) ? 1 : 0;
-        }
+        // Tasks of the step (step_plan), dealt round-robin to the warps, waves first
+        const uint32_t plan = s.plan[D];
+        const int ntw = (int)(plan & 0xffu), nE = (int)((plan >> 8) & 0xffu), Afirst = (int)((plan >> 16) & 3u), lp = (int)(plan >> 20);
+        const int D0 = D + 1, elen = D0 - 3;
         uint32_t *part = s.val + NT * C::VPITCH;
         const int ntask = ntw + (nE << lp);
         for (int t = warp; t < ntask; t += C::NWARP) {

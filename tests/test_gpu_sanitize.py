@@ -3,7 +3,7 @@ SURVEY.md section 4 tier (vi)); profiles/r02_sanitizer.md holds the commands and
 
     compute-sanitizer --tool <tool> python -m pytest tests/test_gpu_sanitize.py -m gpu -x -q
 
-Small n (<= 3T), q = 4, 8, 10, full tables and one ragged batch, every result against the oracle."""
+Small n (<= 3T), q = 4, 8, 10, full tables and one ragged batch on every engine, every result against the oracle."""
 import numpy as np
 import pytest
 
@@ -31,7 +31,17 @@ def test_small_folds_and_one_batch(q):
         assert int(score.item()) == want_score and (tab.cpu().numpy() == want).all(), (q, n)
     seqs, _ = workloads.random_sequences(41 + q, 6, 0, 2 * T + 5)
     flat, offsets, lens = workloads.pack_batch(seqs)
-    got = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens)
-    torch.cuda.synchronize()
-    assert (got.cpu().numpy() == np.array([oracle.nussinov(x) for x in seqs])).all()
+    want = np.array([oracle.nussinov(x) for x in seqs])
+    for eng in (pkg.ENGINE_AUTO, pkg.ENGINE_TILED):        # AUTO: the batch runs on the SMEM engine when q is in 4..8
+        r.set_engine(eng)
+        got = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens)
+        torch.cuda.synchronize()
+        assert (got.cpu().numpy() == want).all(), (q, eng)
+    if q <= 8:                                              # the SMEM engine's single fold with the table
+        r.set_engine(pkg.ENGINE_SMEM)
+        s = seqs[-1] if len(seqs[-1]) else b"ACGU" * 9
+        want_score, want_tab = oracle.nussinov(s, want_table=True)
+        score, tab = r.fold(torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda(), table_dtype=pkg.TABLE_INT32)
+        torch.cuda.synchronize()
+        assert int(score.item()) == want_score and (tab.cpu().numpy() == want_tab).all()
     r.close()

@@ -28,13 +28,14 @@ def dev(s: bytes):
 
 
 def test_two_streams_back_to_back(rna):
-    """cfg4 batch x 200 on one stream while cfg3 x 50 runs on another (separate contexts and workspaces)."""
+    """cfg4 batch x 200 on one stream (tiled engine: the flag protocol; then the SMEM engine a user's AUTO call takes)
+    while cfg3 x 50 runs on another (separate contexts and workspaces)."""
     seqs, lens = workloads.gc_rich_batch()
     want4 = np.loadtxt(os.path.join(GOLD, "cfg4_scores.txt"), dtype=np.int64, comments="#")[:, 2]
     flat, offsets, lens32 = workloads.pack_batch(seqs)
     s3 = workloads.single_config("cfg3")
     want3 = 2761                                   # tests/golden/cfg3_expected.txt (SURVEY 8(c) p9)
-    ra, rb = rna.Rna4r(8, 0), rna.Rna4r(8, 0)
+    ra, rb = rna.Rna4r(8, 0, rna.ENGINE_TILED), rna.Rna4r(8, 0)
     sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
     fd, od, d3 = torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), dev(s3)
     wsa = torch.empty(ra.workspace_bytes_batch(lens32), dtype=torch.uint8, device="cuda")
@@ -56,6 +57,16 @@ def test_two_streams_back_to_back(rna):
     got4 = outa.cpu().numpy()
     assert (got4 == want4[None, :]).all(), np.argwhere(got4 != want4[None, :])[:5]
     assert (outb.cpu().numpy() == want3).all()
+    ra.set_engine(rna.ENGINE_AUTO)
+    outa.fill_(-7)
+    for ia in range(NA):
+        ra.fold_batch(fd, od, lens32, scores_out=outa[ia], workspace=wsa, stream=sa)
+        if ia % 8 == 0:
+            rb.fold(d3, score_out=outb[ia // 8:ia // 8 + 1], workspace=wsb, stream=sb)
+    torch.cuda.synchronize()
+    assert ra.last_launch_count() == 1
+    assert (outa.cpu().numpy() == want4[None, :]).all()
+    assert (outb.cpu().numpy() == want3).all()
     ra.close()
     rb.close()
 
@@ -64,7 +75,7 @@ def test_two_streams_back_to_back(rna):
 def test_every_grid_size(rna, q):
     """the task list is claimed in order and a claimed task only waits on earlier ones: any grid completes and
     gives the same table -- 1, 2, 3, 7 CTAs in all, then 1..3 CTAs per SM"""
-    r = rna.Rna4r(q, 0)
+    r = rna.Rna4r(q, 0, rna.ENGINE_TILED)
     T = 8 * q
     rs = np.random.RandomState(900 + q)
     s = bytes(np.frombuffer(b"ACGU", dtype=np.uint8)[rs.randint(0, 4, size=5 * T + 11)])
