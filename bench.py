@@ -134,6 +134,20 @@ def cpu_baselines(seq: bytes, q: int):
             "score": tv["score"],
         }
     }
+    # the paper's speed-up table (Nussinov seconds and the speed-ups of two-vector, partially
+    # memoised, completely memoised, FG) on this host, on the same 3000-base sample as the oracle above
+    tab = {"n": n_s, "nussinov_s": dt, "paper_row_n3000": {"nussinov_s": 62.5, "two_vector": 8.8, "partially_memoized": 8.3,
+                                                            "completely_memoized": 6.4, "frid_gusfield": 3.4, "cite": "PAPER.md:320"}}
+    for name, qq, fn in (("two_vector", q, lambda: oracle.two_vector_serial(seq[:n_s], q)),
+                         ("partially_memoized", q, lambda: oracle.serial_variant(seq[:n_s], q, "partially_memoized")),
+                         ("completely_memoized", q, lambda: oracle.serial_variant(seq[:n_s], q, "completely_memoized")),
+                         ("frid_gusfield", 3, lambda: oracle.serial_variant(seq[:n_s], 3, "frid_gusfield"))):
+        t0 = time.perf_counter()
+        rr = fn()
+        dtv = time.perf_counter() - t0
+        assert rr["score"] == sc
+        tab[name] = {"q": qq, "seconds": dtv, "speedup_vs_nussinov": dt / dtv}
+    extra["serial_speedup_table"] = tab
     return base, extra
 
 
@@ -173,7 +187,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-also", action="store_true", help="skip the extra workloads (cfg2, cfg4 batch, cfg5)")
     ap.add_argument("--profile", action="store_true", help="short run for ncu: no e2e leg, no tail loop, no extras")
-    ap.add_argument("--engine", default="tiled", choices=["tiled", "diag"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "tiled", "diag"],
+                    help="auto (what a user gets): single folds on the tiled engine, batches of short sequences on the "
+                         "CTA-per-sequence shared-memory engine")
     ap.add_argument("--cfg", default="cfg3", choices=["cfg2", "cfg3", "cfg5"],
                     help="single-sequence workload (profiling aid; the headline and the default is cfg3)")
     args = ap.parse_args()
@@ -214,7 +230,7 @@ def main():
     # one-time preprocessing (step a2), timed separately
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    r = pkg.Rna4r(Q, local_rank, pkg.ENGINE_TILED if args.engine == "tiled" else pkg.ENGINE_DIAG)
+    r = pkg.Rna4r(Q, local_rank, {"auto": pkg.ENGINE_AUTO, "tiled": pkg.ENGINE_TILED, "diag": pkg.ENGINE_DIAG}[args.engine])
     torch.cuda.synchronize()
     prepare_ms = (time.perf_counter() - t0) * 1e3
     r.enable_kernel_timing(True)
@@ -300,7 +316,7 @@ def main():
     ach_lookups = L_lookups / (fill_avg_ms * 1e-3)
     alg_bytes = n + 4                                                  # read n bases, write one int32 score
     roofline = {
-        "bound": "smem", "kernel": "tiled::fill_kernel<8>" if args.engine == "tiled" else "diag_fill_kernel (all diagonals)",
+        "bound": "smem", "kernel": "tiled::fill_kernel<8>" if args.engine != "diag" else "diag_fill_kernel (all diagonals)",
         "achieved": ach_lookups / 1e9, "peak": peak_lookups / 1e9, "unit": "Glookup/s",
         "frac": ach_lookups / peak_lookups,
         "traffic": None,
@@ -315,7 +331,7 @@ def main():
     # DRAM traffic of the same kernel, per launch: an ncu counter cannot be read inside an un-profiled run, so this
     # is the committed value of the latest `ncu --set full` capture (profiles/traffic.json names the capture)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath) and CFG == "cfg3" and args.engine == "tiled":
+    if os.path.exists(tpath) and CFG == "cfg3" and args.engine != "diag":
         try:
             with open(tpath) as f:
                 tj = json.load(f)
@@ -325,7 +341,7 @@ def main():
             pass
     # measured ceiling of the lookup sequence itself (rna4r_microbench_lookups): what the SM sustains for the bare
     # 4-instruction lookup, and for the bulk product's inner loop, conflict-free on every SM
-    if not args.profile and args.engine == "tiled":
+    if not args.profile and args.engine != "diag":
         try:
             ceil = {}
             for name, variant in (("pure_4_instr_lookup", 0), ("bulk_product_inner_loop", 1)):
@@ -345,7 +361,7 @@ def main():
         "fold_time_s": ms_per_step * 1e-3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "n": n, "q": Q, "engine": args.engine, "score": score,
+        "config": {"workload": WORKLOAD, "n": n, "q": Q, "engine": {1: "tiled", 2: "diag", 3: "smem"}[r.engine], "score": score,
                    "l2": "flushed between steps (256 MB write)", "prepare": "rna4r_prepare timed separately (prepare_ms)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "prepare_ms": prepare_ms,
@@ -460,7 +476,14 @@ def also_workloads(pkg, torch, r8, flush):
     wtot = int(sum(nussinov_updates(int(x)) for x in lens32))
     ltot = int(sum(algorithmic_lookups(int(x), 8) for x in lens32))
     res["cfg4_batch1024_q8"] = {"ms": ms, "cell_k_updates_per_s": wtot / (ms * 1e-3), "fill_kernel_ms": r8.last_fill_kernel_ms(),
-                               "lookups": ltot, "sum_scores": int(sc.sum().item())}
+                               "lookups": ltot, "sum_scores": int(sc.sum().item()),
+                               "engine": "smem (one CTA per sequence, one launch)" if r8.last_launch_count() == 1 else "tiled",
+                               "kernel": "smemseq::seq_kernel<8,false>" if r8.last_launch_count() == 1 else "tiled::fill_kernel<8>"}
+    # the same batch forced onto the long-sequence (tiled) engine: what the batch cost before the SMEM engine existed
+    if r8.last_launch_count() == 1:
+        rt = pkg.Rna4r(8, 0, pkg.ENGINE_TILED)
+        res["cfg4_batch1024_q8"]["tiled_engine_ms"] = time_call(lambda: rt.fold_batch(fd, od, lens32, scores_out=sc, workspace=wsb), 5)
+        rt.close()
     del wsb
     # the same batch end to end: pinned host buffers through rna4r_fold_batch_host, copies inside the timed region
     pinned = torch.from_numpy(flat).pin_memory()

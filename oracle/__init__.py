@@ -9,6 +9,8 @@ Functions and the passages they follow:
   brute_force_matchings / brute_force_structural -- the definition, PAPER.md:45     (the pins)
   blackbox / rtable                             -- listing PAPER.md:91-113          (pinned)
   two_vector_serial                             -- Algorithm 1, PAPER.md:125-187    (baseline, pinned to eq. (1))
+  serial_variant                                -- partially / completely memoised and Frid-Gusfield variants,
+                                                   PAPER.md:199-219                 (baselines, pinned to eq. (1))
   structure.check_structure / structure.traceback -- feasibility by the definition; plain
                                                    traceback of eq. (1), PAPER.md:54, :87 (pinned)
 """
@@ -38,6 +40,7 @@ def lib():
         L.oracle_blackbox.argtypes = [ctypes.c_int, ctypes.c_uint32, ctypes.c_uint32, ctypes.POINTER(ctypes.c_int)]
         L.oracle_rtable.argtypes = [ctypes.c_int, u8p]
         L.oracle_two_vector_serial.argtypes = [ctypes.c_char_p, ctypes.c_int, ctypes.c_int, i32p, i64p]
+        L.oracle_serial_variant.argtypes = [ctypes.c_char_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, i64p]
         L.oracle_validate.argtypes = [ctypes.c_char_p, ctypes.c_int]
     return _lib
 
@@ -123,3 +126,19 @@ def two_vector_serial(seq, q: int, want_table: bool = False):
     lk = ctypes.c_int64(0)
     r = lib().oracle_two_vector_serial(s, n, q, _p(tab, ctypes.c_int32) if want_table and n else None, ctypes.byref(lk))
     return {"score": r, "table": tab, "lookups": lk.value}
+
+
+SERIAL_VARIANTS = {"partially_memoized": 1, "completely_memoized": 2, "frid_gusfield": 3}
+
+
+def serial_variant(seq, q: int, variant: str, want_table: bool = False):
+    """The paper's other serial variants: 'partially_memoized', 'completely_memoized',
+    'frid_gusfield'.  Returns dict(score=, table=, lookups=, blackbox_evals=, table_bytes=)."""
+    s = _as_bytes(seq)
+    n = len(s)
+    tab = np.zeros((n, n), dtype=np.int32) if want_table else None
+    st = (ctypes.c_int64 * 3)()
+    r = lib().oracle_serial_variant(s, n, q, SERIAL_VARIANTS[variant], _p(tab, ctypes.c_int32) if want_table and n else None, st)
+    if r == -2:
+        raise MemoryError("serial_variant: out of memory")
+    return {"score": r, "table": tab, "lookups": st[0], "blackbox_evals": st[1], "table_bytes": st[2]}

@@ -5,7 +5,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["nussinov.c", "brute_force.c", "rtable.c", "two_vector_serial.c"]
+SOURCES = ["nussinov.c", "brute_force.c", "rtable.c", "two_vector_serial.c", "serial_variants.c"]
 LIB = os.path.join(HERE, "liboracle.so")
 
 

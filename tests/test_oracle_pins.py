@@ -209,6 +209,39 @@ def test_p8_algorithm1_equals_plain_random_to_600():
         assert r["lookups"] > 0
 
 
+# ---------------------------------------------------------------- p8': the other serial variants
+@pytest.mark.parametrize("variant", ["partially_memoized", "completely_memoized", "frid_gusfield"])
+@pytest.mark.parametrize("q", [2, 3, 4, 5, 8])
+def test_p8_serial_variants_equal_plain_all_small_n(variant, q):
+    rs = np.random.RandomState(85 + q)
+    for n in range(0, 3 * q + 3):
+        s = rand_seq(rs, n)
+        a, ta = oracle.nussinov(s, want_table=True)
+        r = oracle.serial_variant(s, q, variant, want_table=True)
+        assert r["score"] == a, (variant, q, n, s)
+        assert (r["table"] == ta).all(), (variant, q, n, s)
+
+
+def test_p8_serial_variants_random_and_preprocessing_work():
+    """whole tables against eq. (1); the memoised variants preprocess no more than the exhaustive 2^2q pairs
+    (PAPER.md:219), the completely memoised one no more than the partially memoised one, and FG does
+    2^q evaluations for every group of every row ("duplicated work")"""
+    rs = np.random.RandomState(86)
+    for q, n in ((3, 211), (4, 256), (5, 333), (8, 500)):
+        s = rand_seq(rs, n)
+        a, ta = oracle.nussinov(s, want_table=True)
+        res = {v: oracle.serial_variant(s, q, v, want_table=True) for v in oracle.SERIAL_VARIANTS}
+        tv = oracle.two_vector_serial(s, q)
+        for v, r in res.items():
+            assert r["score"] == a and (r["table"] == ta).all(), (v, q, n)
+            assert r["lookups"] == tv["lookups"]
+        pm, cm, fg = res["partially_memoized"], res["completely_memoized"], res["frid_gusfield"]
+        assert 0 < cm["blackbox_evals"] <= pm["blackbox_evals"] <= 4 ** q
+        assert pm["blackbox_evals"] % (1 << q) == 0
+        assert fg["blackbox_evals"] > pm["blackbox_evals"] and fg["blackbox_evals"] % (1 << q) == 0
+    assert oracle.serial_variant(b"ACGN", 4, "frid_gusfield")["score"] == -1
+
+
 # ---------------------------------------------------------------- p7: R table
 @pytest.mark.parametrize("q", [2, 3, 4, 5, 8, 10])
 def test_p7_rtable_pins(q):
