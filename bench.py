@@ -466,6 +466,15 @@ def also_workloads(pkg, torch, r8, flush):
         if q != 8:
             rq.close()
     res["q_sweep_n6000_ms"] = sweep
+    # the comparison engines at n = 6000, q = 8: the paper's section 4 kernel (one launch per cell
+    # diagonal), its section 5.3 q x q tile kernel (one launch per tile diagonal), and a DPX max-plus kernel without R
+    cmp_ms = {"tiled": sweep["8"]}
+    for name, eng in (("diag_paper_section4", pkg.ENGINE_DIAG), ("paper_tile_section5_3", pkg.ENGINE_PAPER_TILE),
+                      ("maxplus_dpx_no_table", pkg.ENGINE_MAXPLUS)):
+        rc = pkg.Rna4r(8, 0, eng)
+        cmp_ms[name] = time_call(lambda: rc.fold(d3), 2)
+        rc.close()
+    res["engines_n6000_q8_ms"] = cmp_ms
     # cfg4 batch
     seqs, lens = workloads.gc_rich_batch()
     flat, offsets, lens32 = workloads.pack_batch(seqs)

@@ -88,6 +88,14 @@ extern "C" {
                                      in shared memory (batches of short sequences, BASELINE.json
                                      configs[3]); q in 4..8, n <= rna4r_smem_max_n */
 
+#define RNA4R_ENGINE_PAPER_TILE 4  /* the paper's own CUDA design, section 5.3: one block per
+                                     q x q tile, one launch per tile-diagonal, only differences (+ anchors)
+                                     stored, H vectors row-major by tile, V vectors column-major by tile, R in
+                                     global memory; any q in 2..12; a comparison point                       */
+#define RNA4R_ENGINE_MAXPLUS 5    /* no Four-Russians table: eq. (1) as a blocked max-plus
+                                     closure on int16 values with DPX add-max, one launch per 32 x 32 tile-
+                                     diagonal; q is ignored; a comparison point           */
+
 typedef struct rna4r_ctx rna4r_ctx;   /* opaque; owns the device R tables for one q on one device */
 
 /*

@@ -4,8 +4,8 @@ The product is the C-ABI shared library `librna4r.so` (include/rna4r.h) built fr
 for sm_100a; this package is its thin Python binding (argument marshalling only).
 """
 from . import shard
-from .binding import (ENGINE_AUTO, ENGINE_DIAG, ENGINE_SMEM, ENGINE_TILED, TABLE_INT16, TABLE_INT32, TABLE_NONE, Rna4r, Rna4rError,
+from .binding import (ENGINE_AUTO, ENGINE_DIAG, ENGINE_MAXPLUS, ENGINE_PAPER_TILE, ENGINE_SMEM, ENGINE_TILED, TABLE_INT16, TABLE_INT32, TABLE_NONE, Rna4r, Rna4rError,
                       load, rna4r_prepare)
 
 __all__ = ["Rna4r", "Rna4rError", "rna4r_prepare", "load", "TABLE_NONE", "TABLE_INT16", "TABLE_INT32",
-           "ENGINE_AUTO", "ENGINE_TILED", "ENGINE_DIAG", "ENGINE_SMEM", "shard"]
+           "ENGINE_AUTO", "ENGINE_TILED", "ENGINE_DIAG", "ENGINE_SMEM", "ENGINE_PAPER_TILE", "ENGINE_MAXPLUS", "shard"]

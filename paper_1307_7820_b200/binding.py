@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 TABLE_NONE, TABLE_INT16, TABLE_INT32 = 0, 1, 2
-ENGINE_AUTO, ENGINE_TILED, ENGINE_DIAG, ENGINE_SMEM = 0, 1, 2, 3
+ENGINE_AUTO, ENGINE_TILED, ENGINE_DIAG, ENGINE_SMEM, ENGINE_PAPER_TILE, ENGINE_MAXPLUS = 0, 1, 2, 3, 4, 5
 
 _lib = None
 

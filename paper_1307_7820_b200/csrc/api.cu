@@ -5,6 +5,7 @@
 #include "diag_engine.cuh"
 #include "tiled_engine.cuh"
 #include "smem_engine.cuh"
+#include "compare_engines.cuh"
 #include "traceback.cuh"
 #include "microbench.cuh"
 
@@ -72,13 +73,31 @@ inline int smem_max_n(int q)
     }
 }
 
+// the engines that fold one sequence per call (the comparison engines): workspace of one fold, and the enqueue
+inline bool per_sequence_engine(int e) { return e == RNA4R_ENGINE_DIAG || e == RNA4R_ENGINE_PAPER_TILE || e == RNA4R_ENGINE_MAXPLUS; }
+size_t single_ws(const rna4r_ctx *ctx, int n)
+{
+    if (ctx->engine == RNA4R_ENGINE_PAPER_TILE) return cmpeng::pt_layout(nullptr, n, ctx->q).bytes;
+    if (ctx->engine == RNA4R_ENGINE_MAXPLUS) return cmpeng::mp_layout(nullptr, n).bytes;
+    return diag_ws_layout(nullptr, n).bytes;
+}
+int single_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, const int64_t *offset_dev, int n, int32_t *score_dev, int32_t *status_dev,
+                   void *table_out, int table_dtype, void *ws, cudaStream_t st)
+{
+    if (ctx->engine == RNA4R_ENGINE_PAPER_TILE)
+        return cmpeng::pt_fold_enqueue(ctx, seq_dev, offset_dev, n, score_dev, status_dev, table_out, table_dtype, ws, st);
+    if (ctx->engine == RNA4R_ENGINE_MAXPLUS)
+        return cmpeng::mp_fold_enqueue(ctx, seq_dev, offset_dev, n, score_dev, status_dev, table_out, table_dtype, ws, st);
+    return diag_fold_enqueue(ctx, seq_dev, offset_dev, n, score_dev, status_dev, table_out, table_dtype, ws, st);
+}
+
 size_t engine_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_single)
 {
     if (ctx->engine == RNA4R_ENGINE_SMEM) return smemseq::workspace_bytes(count);
     if (ctx->engine == RNA4R_ENGINE_TILED) return tiled_ws(ctx, lens, count, n_single);
-    // DIAG: sequences of a batch are folded one after another, each in its own slice
+    // per-sequence engines: sequences of a batch are folded one after another, each in its own slice
     size_t total = 0;
-    for (int t = 0; t < count; ++t) total += diag_ws_layout(nullptr, lens ? lens[t] : n_single).bytes;
+    for (int t = 0; t < count; ++t) total += single_ws(ctx, lens ? lens[t] : n_single);
     return total;
 }
 
@@ -248,7 +267,7 @@ int rna4r_set_engine(rna4r_ctx *ctx, int engine)
     if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
     const int is_auto = engine == RNA4R_ENGINE_AUTO;
     if (is_auto) engine = (ctx->q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
-    if (engine != RNA4R_ENGINE_TILED && engine != RNA4R_ENGINE_DIAG && engine != RNA4R_ENGINE_SMEM) return RNA4R_ERR_ENGINE;
+    if (engine != RNA4R_ENGINE_TILED && engine != RNA4R_ENGINE_SMEM && !per_sequence_engine(engine)) return RNA4R_ERR_ENGINE;
     if (engine == RNA4R_ENGINE_TILED && ctx->q > 10) return RNA4R_ERR_ENGINE;
     if (engine == RNA4R_ENGINE_SMEM && !smem_q_ok(ctx->q)) return RNA4R_ERR_ENGINE;
     ctx->engine = engine;
@@ -283,7 +302,7 @@ size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count, int fla
         // every sequence at n_max: per-sequence cost is monotone in n
         if (ctx->engine == RNA4R_ENGINE_TILED) core = (size_t)count * tiled_ws(ctx, nullptr, 1, n_max);
         else if (ctx->engine == RNA4R_ENGINE_SMEM) core = smemseq::workspace_bytes(count);
-        else core = (size_t)count * diag_ws_layout(nullptr, n_max).bytes;
+        else core = (size_t)count * single_ws(ctx, n_max);
     }
     if (!(flags & (RNA4R_WS_HOST_STAGING | RNA4R_WS_HOST_TABLE16 | RNA4R_WS_HOST_TABLE32))) return core;
     size_t table_bytes = 0;
@@ -318,6 +337,8 @@ int rna4r_fold(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_out
         const size_t es = table_dtype == RNA4R_TABLE_INT16 ? 2 : 4;
         RNA4R_CUDA(ctx, cudaMemsetAsync(table_out_dev, 0, (size_t)n * n * es, st));   // zeros below the diagonal
     }
+    if (per_sequence_engine(ctx->engine))      // PAPER_TILE / MAXPLUS (DIAG returned above: it writes the whole table itself)
+        return single_enqueue(ctx, seq_dev, nullptr, n, score_out_dev, nullptr, table_out_dev, table_dtype, workspace_dev, st);
     if (ctx->engine == RNA4R_ENGINE_SMEM)
         return dispatch_q_smem(ctx->q, [&](auto Q) {
             return smemseq::enqueue_q<decltype(Q)::value>(ctx, seq_dev, nullptr, nullptr, 1, n, score_out_dev, nullptr, table_out_dev,
@@ -354,16 +375,16 @@ int rna4r_fold_batch_status(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64
     if (workspace_bytes < engine_ws(ctx, lens_host, count, 0)) return RNA4R_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (ctx->engine == RNA4R_ENGINE_DIAG) {
+    if (per_sequence_engine(ctx->engine)) {
         size_t ws_off = 0;            // sequence t starts at offsets_dev[t] (read on the device)
         int launches = 0;
         for (int t = 0; t < count; ++t) {
-            int rc = diag_fold_enqueue(ctx, seqs_dev, offsets_dev + t, lens_host[t], scores_out_dev + t,
-                                       status_out_dev ? status_out_dev + t : nullptr, nullptr, RNA4R_TABLE_NONE,
-                                       (char *)workspace_dev + ws_off, st);
+            int rc = single_enqueue(ctx, seqs_dev, offsets_dev + t, lens_host[t], scores_out_dev + t,
+                                    status_out_dev ? status_out_dev + t : nullptr, nullptr, RNA4R_TABLE_NONE,
+                                    (char *)workspace_dev + ws_off, st);
             if (rc != RNA4R_OK) return rc;
             launches += ctx->last_launches;
-            ws_off += diag_ws_layout(nullptr, lens_host[t]).bytes;
+            ws_off += single_ws(ctx, lens_host[t]);
         }
         ctx->last_launches = launches;
         return RNA4R_OK;

@@ -60,11 +60,12 @@ def test_rtable_entry_by_entry(rna, q):
 
 
 # ------------------------------------------------------------------ full-table parity, small n
-ENGINES = ["tiled", "diag"]
+ENGINES = ["tiled", "diag", "paper_tile", "maxplus"]
 
 
 def engine_id(pkg, name):
-    return pkg.ENGINE_TILED if name == "tiled" else pkg.ENGINE_DIAG
+    return {"tiled": pkg.ENGINE_TILED, "diag": pkg.ENGINE_DIAG, "paper_tile": pkg.ENGINE_PAPER_TILE,
+            "maxplus": pkg.ENGINE_MAXPLUS}[name]
 
 
 @pytest.mark.parametrize("engine", ENGINES)
@@ -143,7 +144,7 @@ def read_expected(name):
 def test_cfg1_full_table_q4_int32(rna):
     s = workloads.single_config("cfg1")
     want_score, want = oracle.nussinov(s, want_table=True)
-    for eng in (rna.ENGINE_TILED, rna.ENGINE_DIAG):
+    for eng in (rna.ENGINE_TILED, rna.ENGINE_DIAG, rna.ENGINE_PAPER_TILE, rna.ENGINE_MAXPLUS, rna.ENGINE_SMEM):
         r = ctx(rna, 4, eng)
         got_score, got = gpu_table(rna, r, s, rna.TABLE_INT32)
         assert got_score == want_score == 110
@@ -155,7 +156,7 @@ def test_cfg2_n2000_q8(rna):
     res = oracle.nussinov_fast(s, threads=os.cpu_count() or 1, want_table=True)
     exp, cells = read_expected("cfg2")
     assert res["score"] == int(exp["score"])
-    for eng in (rna.ENGINE_TILED, rna.ENGINE_DIAG):
+    for eng in (rna.ENGINE_TILED, rna.ENGINE_DIAG, rna.ENGINE_PAPER_TILE, rna.ENGINE_MAXPLUS):
         r = ctx(rna, 8, eng)
         got_score, got = gpu_table(rna, r, s, rna.TABLE_INT16)
         assert got_score == res["score"]
@@ -207,8 +208,9 @@ def test_cfg3_full_table_elementwise(rna):
     assert torch.equal(tab, want), int((tab != want).sum().item())
 
 
-def test_cfg3_n6000_q8_diag_engine(rna):
-    check_large(rna, "cfg3", 8, rna.ENGINE_DIAG)
+@pytest.mark.parametrize("engine", ["diag", "paper_tile", "maxplus"])
+def test_cfg3_n6000_q8_comparison_engines(rna, engine):
+    check_large(rna, "cfg3", 8, engine_id(rna, engine))
 
 
 @pytest.mark.parametrize("q", [8, 10])
