@@ -190,10 +190,14 @@ def main():
     ap.add_argument("--engine", default="auto", choices=["auto", "tiled", "diag"],
                     help="auto (what a user gets): single folds on the tiled engine, batches of short sequences on the "
                          "CTA-per-sequence shared-memory engine")
-    ap.add_argument("--cfg", default="cfg3", choices=["cfg2", "cfg3", "cfg5"],
-                    help="single-sequence workload (profiling aid; the headline and the default is cfg3)")
+    ap.add_argument("--cfg", default="cfg3", choices=["cfg2", "cfg3", "cfg4", "cfg5"],
+                    help="workload (profiling aid; the headline and the default is cfg3; cfg4 = the batch, device-timed only)")
+    ap.add_argument("--q", type=int, default=8, help="vector length q (profiling aid; the headline is q = 8)")
     args = ap.parse_args()
-    global CFG, WORKLOAD
+    global CFG, WORKLOAD, Q
+    Q = args.q
+    if args.cfg == "cfg4":
+        return profile_batch(args)
     if args.cfg != CFG:
         CFG = args.cfg
         WORKLOAD = f"{CFG}: single RNA sequence n={workloads.SINGLE_CONFIGS[CFG]['n']}, i.i.d. uniform {{A,C,G,U}}, q=8, score only"
@@ -316,7 +320,7 @@ def main():
     ach_lookups = L_lookups / (fill_avg_ms * 1e-3)
     alg_bytes = n + 4                                                  # read n bases, write one int32 score
     roofline = {
-        "bound": "smem", "kernel": "tiled::fill_kernel<8>" if args.engine != "diag" else "diag_fill_kernel (all diagonals)",
+        "bound": "smem", "kernel": f"tiled::fill_kernel<{Q}>" if args.engine != "diag" else "diag_fill_kernel (all diagonals)",
         "achieved": ach_lookups / 1e9, "peak": peak_lookups / 1e9, "unit": "Glookup/s",
         "frac": ach_lookups / peak_lookups,
         "traffic": None,
@@ -331,7 +335,7 @@ def main():
     # DRAM traffic of the same kernel, per launch: an ncu counter cannot be read inside an un-profiled run, so this
     # is the committed value of the latest `ncu --set full` capture (profiles/traffic.json names the capture)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath) and CFG == "cfg3" and args.engine != "diag":
+    if os.path.exists(tpath) and CFG == "cfg3" and Q == 8 and args.engine != "diag":
         try:
             with open(tpath) as f:
                 tj = json.load(f)
@@ -341,7 +345,7 @@ def main():
             pass
     # measured ceiling of the lookup sequence itself (rna4r_microbench_lookups): what the SM sustains for the bare
     # 4-instruction lookup, and for the bulk product's inner loop, conflict-free on every SM
-    if not args.profile and args.engine != "diag":
+    if not args.profile and args.engine != "diag" and Q == 8:
         try:
             ceil = {}
             for name, variant in (("pure_4_instr_lookup", 0), ("bulk_product_inner_loop", 1)):
@@ -389,6 +393,28 @@ def main():
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def profile_batch(args):
+    """--cfg cfg4: the batch of config 4 through rna4r_fold_batch (AUTO: the SMEM engine), device-timed; for ncu."""
+    import torch
+    import paper_1307_7820_b200 as pkg
+    r = pkg.Rna4r(Q, 0, {"auto": pkg.ENGINE_AUTO, "tiled": pkg.ENGINE_TILED, "diag": pkg.ENGINE_DIAG}[args.engine])
+    r.enable_kernel_timing(True)
+    seqs, lens = workloads.gc_rich_batch()
+    flat, offsets, lens32 = workloads.pack_batch(seqs)
+    fd, od = torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda()
+    ws = torch.empty(r.workspace_bytes_batch(lens32), dtype=torch.uint8, device="cuda")
+    sc = torch.empty(len(lens32), dtype=torch.int32, device="cuda")
+    ms = []
+    for _ in range(max(args.warmup, 1) + args.steps):
+        r.fold_batch(fd, od, lens32, scores_out=sc, workspace=ws)
+        ms.append(r.last_fill_kernel_ms())
+    ltot = int(sum(algorithmic_lookups(int(x), Q) for x in lens32))
+    k = float(np.median(ms[max(args.warmup, 1):]))
+    print(json.dumps({"workload": "cfg4: 1024 sequences, lengths U[300,700], one rna4r_fold_batch call", "q": Q,
+                      "launches_per_call": r.last_launch_count(), "kernel_ms": k, "lookups": ltot,
+                      "smem_roofline_frac": ltot / (k * 1e-3) / (148 * 32 * 1.965e9), "sum_scores": int(sc.sum().item())}))
 
 
 def sharded_batch(pkg, torch, dist, r, rank, world, barrier, steps):

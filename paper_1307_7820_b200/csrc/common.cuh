@@ -35,6 +35,16 @@ struct rna4r_ctx {
 #endif
 static const uint32_t RNA4R_MAGIC = 0x52344e41u;
 
+// Checked build (-DRNA4R_CHECKS; tests and profiles/r02_sanitizer.md): every freshly computed cell must differ from its
+// finished neighbours by 0 or 1 (Lemma 1), packed offsets must fit their fields and table indices the
+// table.  A cell computed from operands that another warp / CTA had not finished yet breaks Lemma 1 with high
+// probability, so this traps on ordering bugs of the flag / barrier protocols as well as on out-of-range indices.
+#ifdef RNA4R_CHECKS
+#define RNA4R_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define RNA4R_CHECK(cond) do { } while (0)
+#endif
+
 #define RNA4R_CUDA(ctx, call)                                             \
     do {                                                                  \
         cudaError_t e__ = (call);                                         \

@@ -149,6 +149,7 @@ __device__ __forceinline__ uint32_t lookup_max(uint32_t tbl_sa, uint32_t S, uint
 {
     uint32_t rv;
     asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"((S >> Cfg<Q>::ISH) + tbl_sa));
+    RNA4R_CHECK((S >> Cfg<Q>::ISH) < (uint32_t)Cfg<Q>::TBL_BYTES && (S & 0xffffu) + rv < (1u << Cfg<Q>::VBITS));
     return __viaddmax_u16x2(S, rv, acc);
 }
 
@@ -195,7 +196,10 @@ __device__ __forceinline__ uint32_t pack_rows(const uint32_t (&acc)[Q])
     const uint32_t base = acc[Q - 1] & 0xffffu;
     uint32_t w = base;
 #pragma unroll
-    for (int a = 0; a < Q - 1; ++a) w |= (((acc[a] & 0xffffu) - base) & 7u) << (Cfg<Q>::VBITS + 3 * a);
+    for (int a = 0; a < Q - 1; ++a) {
+        RNA4R_CHECK((acc[a] & 0xffffu) - base <= 7u && base < (1u << Cfg<Q>::VBITS));
+        w |= (((acc[a] & 0xffffu) - base) & 7u) << (Cfg<Q>::VBITS + 3 * a);
+    }
     return w;
 }
 template <int Q>
@@ -407,6 +411,7 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
         v = max((int)(short)(m2 & 0xffff), m2 >> 16);
         // ---- step a6: row word of row r over group B (ballot of the horizontal differences), column word bit
         vl = __shfl_sync(FULL, v, lane - 1);
+        RNA4R_CHECK(!own || ((unsigned)(v - vprev) <= 1u && (y == 0 || (unsigned)(v - vl) <= 1u)));   // Lemma 1
         const uint32_t bal = __ballot_sync(FULL, y > 0 && v != vl);
         wout[a] = (((bal >> bsh) & C::HMASK) << 24) | (uint32_t)v;
         rlo[a] = (int16_t)v;

@@ -693,6 +693,7 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         if (s + 1 < Q && y == s + 1) v = vbelow;                    // pre-step (x = -1): the cell below the q-tile
         if (MERGED && s - (Q - 1) <= 1) v = 0;                      // D(i,i) = D(i,i-1) = 0
         const bool live = own && (unsigned)(s - y) < (unsigned)Q;
+        RNA4R_CHECK(!live || ((unsigned)(v - Lv) <= 1u && (s - y == 0 || (unsigned)(v - vprev) <= 1u)));   // Lemma 1 against the left and the lower cell
         if (live) vb[-s * VP] = (int16_t)v;
         // ---- tail lookup of the NEXT cell: row word of row a-1 through column c-2 x column word of group B of block J
         tS = Lw2 + (MERGED ? Xp : XJ);

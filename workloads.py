@@ -23,6 +23,8 @@ SINGLE_CONFIGS = {
     "cfg2": {"seed": 1, "n": 2000, "q": (8,), "table_dtype": "int16"},
     "cfg3": {"seed": 2, "n": 6000, "q": (8,), "table_dtype": "int16"},
     "cfg5": {"seed": 4, "n": 16384, "q": (8, 10), "table_dtype": "int16"},
+    # beyond BASELINE.json's five configs ("n > 16384"): the same recipe at twice the length
+    "cfg6": {"seed": 6, "n": 32768, "q": (8,), "table_dtype": "int16"},
 }
 BATCH_CONFIG = {"seed": 3, "count": 1024, "lo": 300, "hi": 700, "q": (8,)}
 
