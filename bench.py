@@ -543,6 +543,12 @@ def also_workloads(pkg, torch, r8, flush):
         ms = time_call(lambda: rr.fold(d), 3)
         res[f"cfg5_n16384_q{q}"] = {"ms": ms, "cell_k_updates_per_s": nussinov_updates(len(s)) / (ms * 1e-3),
                                     "fill_kernel_ms": rr.last_fill_kernel_ms(), "lookups": algorithmic_lookups(len(s), q)}
+    # cfg6: n = 32768 (beyond BASELINE.json's configs), score only
+    s = workloads.single_config("cfg6")
+    d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()
+    ms = time_call(lambda: r8.fold(d), 2)
+    res["cfg6_n32768_q8"] = {"ms": ms, "cell_k_updates_per_s": nussinov_updates(len(s)) / (ms * 1e-3),
+                             "fill_kernel_ms": r8.last_fill_kernel_ms(), "lookups": algorithmic_lookups(len(s), 8)}
     return res
 
 

@@ -218,6 +218,12 @@ def test_cfg5_n16384(rna, q):
     check_large(rna, "cfg5", q, rna.ENGINE_TILED)
 
 
+def test_cfg6_n32768_q8(rna):
+    """beyond the five configs: n = 32768, score-only call, then the 2 GB int16 table against the
+    oracle's stored cells, table sum and Lemma 1"""
+    check_large(rna, "cfg6", 8, rna.ENGINE_TILED)
+
+
 def test_cfg4_batch_1024(rna):
     seqs, lens = workloads.gc_rich_batch()
     want = np.loadtxt(os.path.join(GOLD, "cfg4_scores.txt"), dtype=np.int64, comments="#")
