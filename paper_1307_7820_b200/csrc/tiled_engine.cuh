@@ -265,6 +265,56 @@ __global__ void encode_kernel(Params p)
     }
 }
 
+// Single fold: the whole plan (geometry, per-step task counts, task list) and the encoding in ONE launch.  Block D owns
+// step D: it sums the task counts of the earlier steps itself (a few hundred terms), writes the step's CLOSE and PROD
+// tasks in the order of the batch path, and encodes the bases of super-tile D.
+template <int Q>
+__global__ void plan_single_kernel(Params p)
+{
+    constexpr int T = Cfg<Q>::T;
+    const int n = p.n_single, nt = n / T + 1;
+    const int D = blockIdx.x, tid = threadIdx.x;
+    auto prods_of = [&](int d) {
+        int np = 0;
+        for (int s = 0;; ++s) {
+            const int dp = d + 1 + s * p.delta;
+            if (dp > nt - 1) break;
+            if (s < nstages(dp, p.delta)) np += nt - dp;
+        }
+        return np;
+    };
+    __shared__ int red[128];
+    int part = 0;
+    for (int d = tid; d < D; d += blockDim.x) part += (nt - d) + prods_of(d);
+    red[tid] = part;
+    __syncthreads();
+    for (int w = blockDim.x / 2; w > 0; w >>= 1) {
+        if (tid < w) red[tid] += red[tid + w];
+        __syncthreads();
+    }
+    const int baseC = red[0], baseP = baseC + (nt - D);
+    for (int I = tid; I < nt - D; I += blockDim.x) p.tasks[baseC + I] = make_int4(0, I | ((I + D) << 16), TASK_CLOSE, 0);
+    int slot = baseP;
+    for (int s = 0;; ++s) {
+        const int dp = D + 1 + s * p.delta;
+        if (dp > nt - 1) break;
+        if (s >= nstages(dp, p.delta)) continue;
+        for (int I = tid; I < nt - dp; I += blockDim.x) p.tasks[slot + I] = make_int4(0, I | ((I + dp) << 16), TASK_PROD, s);
+        slot += nt - dp;
+    }
+    if (tid == 0) {
+        if (D == nt - 1) p.hdr->total = slot;
+        if (D == 0) { SeqInfo *si = p.seqinfo; si->n = n; si->nt = nt; si->sbase = 0; si->cbase = 0; }   // invalid: zeroed, OR-ed below
+    }
+    bool bad = false;
+    for (int x = D * T + tid; x < (D + 1) * T; x += blockDim.x) {
+        int c = 4;
+        if (x < n) { c = rna4r_base_code(p.seqs[x]); bad |= (c == 4); }
+        p.codes[x] = (int8_t)c;
+    }
+    if (bad) atomicOr(&p.seqinfo[0].invalid, RNA4R_STATUS_BAD_BASE);
+}
+
 // ------------------------------------------------------------------------------------------------
 // fill kernel
 // ------------------------------------------------------------------------------------------------
@@ -1350,8 +1400,8 @@ static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int co
     w.off_accstage = off; off += align_up(h.tiles * 4, 256);
     w.off_rowprog = off; off += align_up(h.tiles * 4, 256);
     w.off_colprog = off; off += align_up(h.tiles * 4, 256);
-    w.zero_bytes = off;
     w.off_seqinfo = off; off += align_up((size_t)count * sizeof(SeqInfo), 256);
+    w.zero_bytes = off;
     w.off_lens = off; off += align_up((size_t)count * 4, 256);
     w.off_tasks = off; off += align_up(h.tasks * sizeof(int4), 256);
     w.off_codes = off; off += align_up(h.codes, 256);
@@ -1410,10 +1460,12 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     RNA4R_CUDA(ctx, cudaMemsetAsync(ws, 0, w.zero_bytes, st));
     if (offsets)    // lens_host is consumed before this call returns (pageable memory is staged by the runtime)
         RNA4R_CUDA(ctx, cudaMemcpyAsync(base + w.off_lens, lens_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
-    plan_seq_kernel<Q><<<count, 64, 0, st>>>(p); ++launches;
-    plan_scan_kernel<<<1, 32, 0, st>>>(p); ++launches;
-    plan_fill_kernel<Q><<<count * h.max_nt, 64, 0, st>>>(p); ++launches;
-    {
+    if (!offsets && h.max_nt <= 2048) {
+        plan_single_kernel<Q><<<h.max_nt, 128, 0, st>>>(p); ++launches;          // plan + encode of a single fold: one launch
+    } else {
+        plan_seq_kernel<Q><<<count, 64, 0, st>>>(p); ++launches;
+        plan_scan_kernel<<<1, 32, 0, st>>>(p); ++launches;
+        plan_fill_kernel<Q><<<count * h.max_nt, 64, 0, st>>>(p); ++launches;
         const int maxlen = h.max_nt * C::T;
         dim3 grid((maxlen + 255) / 256, count < 65535 ? count : 65535);
         encode_kernel<Q><<<grid, 256, 0, st>>>(p); ++launches;
