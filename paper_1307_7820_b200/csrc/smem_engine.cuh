@@ -63,13 +63,20 @@ struct Cfg {
     static constexpr int SCR_WARP_HW = 2 * G * 8 + 8 * 2 + 8;    // per-warp scratch in halfwords: row buffers [2][G][8], two dummy store targets
     static constexpr int SCR_BYTES = NWARP * SCR_WARP_HW * 2;
     static constexpr int FIXED_BYTES = TBL_AREA + SCR_BYTES + 64;
+#ifndef RNA4R_SMEM_DATAFLOW
+#define RNA4R_SMEM_DATAFLOW 0
+#endif
+    // Build knob: progress words per tile-row (waves wait for their two neighbours, bulk tasks for a complete diagonal)
+    // instead of the CTA barrier per tile-diagonal.  Measured equal (cfg4 1.60 vs 1.59 ms): the barrier is not what a
+    // sequence waits for, the chain of waves through its neighbours is.
+    static constexpr bool DATAFLOW = RNA4R_SMEM_DATAFLOW != 0;
     static constexpr int MAX_SMEM = 232448;          // 227 KB
 };
 
 // byte offsets of one sequence's state, relative to the start of the pool
 struct Layout {
     int NB;
-    uint32_t W, X, val, wdh, dq, pm, rl, code, plan, total;
+    uint32_t W, X, val, wdh, dq, pm, rl, code, plan, flags, total;
 };
 
 template <int Q>
@@ -89,6 +96,7 @@ __host__ __device__ inline Layout make_layout(int n)
     L.rl = take(2u * Q * NB);
     L.code = take(Q * NB + 16u);
     L.plan = take(4u * NB);
+    L.flags = take(4u * (3u * NB + 8u));
     L.total = off;
     return L;
 }
@@ -137,6 +145,9 @@ struct Sm {
     int16_t *rl;
     int8_t *code;
     uint32_t *plan;           // [NB] step_plan of every tile-diagonal
+    int *prog;                // [NB+1] last tile-diagonal tile-row A has finished          (dataflow schedule)
+    int *bulkd;               // [NB+1] first diagonal D0 of the last strip-tile whose bulk word is in the ring
+    int *cntd;                // [NB+1] finished tiles per tile-diagonal; cntd[NB+1] = last tile-diagonal that is complete
     int n, NB;
 };
 
@@ -326,6 +337,13 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
     const uint16_t *xcol = s.X + off_x<Q>(B) + y;              // xcol[g*Q] = column word of (group g, my column)
     const uint32_t *wrow = s.W + off_w<Q>(NB, A);              // wrow[j*Q + a] = row word of (row r0+a, group A+1+j)
 
+    if constexpr (C::DATAFLOW) {
+        // wait until my tile-row and the one below have finished tile-diagonal D-1 (every other operand of the tile is
+        // older: each tile waited for the tile below it) and the strip-tile's bulk word has been written
+        volatile int *pg = s.prog, *bd = s.bulkd;
+        while (!__all_sync(FULL, pg[A] >= D - 1 && pg[A + 1] >= D - 1 && (D0 < 4 || bd[A] >= D0))) __nanosleep(32);
+        __threadfence_block();
+    }
     // ---- fresh groups (a4): j in [0, min(k, D-2)] (column words of the tiles just below) and from max(D0-2, k+1) to
     // D-2 (row words of the tiles to the left inside the strip); without bulk (D0 < 4) that is every complete group
     uint32_t facc[Q];
@@ -425,6 +443,16 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
         const_cast<uint16_t *>(xcol)[A * Q] = (uint16_t)(((Xp >> C::ISH) << C::XAB) | (Xp & 0xffffu));
         if (A == 0 && c == s.n) p.scores[seq] = v;                // M(0,n) = D(1,n)
     }
+    if constexpr (C::DATAFLOW) {
+        __threadfence_block();
+        __syncwarp();
+        if (own && y == 0) *(volatile int *)(s.prog + A) = D;
+        if (lane == 0) {
+            const int nt4 = min(C::G, (NT - A0 + C::G - 1) / C::G);
+            __threadfence_block();
+            if (atomicAdd(s.cntd + D, nt4) + nt4 == NT) atomicMax(s.cntd + NB + 1, D);                // the diagonal is complete
+        }
+    }
 }
 
 // Plan of tile-diagonal step D: ntw wave tasks | nE bulk tasks << 8 | first tile-row of a bulk task << 16 | log2(parts)
@@ -442,7 +470,7 @@ __device__ __forceinline__ uint32_t step_plan(int NB, int D)
     const int nE = (D0 >= 4 && D0 < NB && NB - 1 - D0 >= Afirst) ? ((NB - 1 - D0 - Afirst) >> 2) + 1 : 0;
     const int elen = D0 - 3;
     int lp = 0;
-    if (nE > 0) {
+    if (nE > 0 && !C::DATAFLOW) {
         const int wfree = C::NWARP - (NT + 3) / 4;
         const int rows = (D * C::VPITCH) / 32;               // part slots (32 words each) the dead rows hold
         lp = (elen >= 72 && 4 * nE <= wfree && 4 * nE <= rows) ? 2 : (elen >= 40 && 2 * nE <= wfree && 2 * nE <= rows) ? 1 : 0;
@@ -469,6 +497,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         s.W = (uint32_t *)(b + L.W); s.X = (uint16_t *)(b + L.X); s.val = (uint32_t *)(b + L.val);
         s.wdh = (uint32_t *)(b + L.wdh); s.dq = b + L.dq; s.pm = b + L.pm; s.rl = (int16_t *)(b + L.rl);
         s.code = (int8_t *)(b + L.code); s.plan = (uint32_t *)(b + L.plan);
+        s.prog = (int *)(b + L.flags); s.bulkd = s.prog + (L.NB + 1); s.cntd = s.bulkd + (L.NB + 1);
         s.n = n; s.NB = L.NB;
         uint32_t dyn;
         asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
@@ -513,6 +542,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         s.pm[e] = (uint8_t)bits;
     }
     for (int D = tid; D < NB; D += C::NTHR) s.plan[D] = step_plan<Q>(NB, D);
+    for (int e = tid; e < 3 * NB + 8; e += C::NTHR) s.prog[e] = 0;
     // ---- tile-diagonal 0
     for (int A = tid; A < NB; A += C::NTHR) diag_tile<Q, TABLE>(p, s, seq, A);
     __syncthreads();
@@ -540,14 +570,26 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
                 uint32_t acc[Q];
 #pragma unroll
                 for (int a = 0; a < Q; ++a) acc[a] = 0;
+                if constexpr (C::DATAFLOW) {
+                    // operands: tiles of the diagonals <= D0-2 = D-1; the ring slots it overwrites were read by tiles of
+                    // tile-row A up to diagonal D0-2 as well
+                    volatile int *ad = s.cntd + NB + 1;
+                    while (*ad < D - 1) __nanosleep(64);
+                    __threadfence_block();
+                }
                 strip_bulk<Q>(s, A, GC, 1 + ((elen * pe) >> lp), (elen * (pe + 1)) >> lp, lane, acc);
                 const uint32_t w = pack_rows<Q>(acc);
                 if (lp > 0) part[e * 32 + lane] = w;
                 else if (lane < C::SW && GC + lane / Q < NB) s.val[val_index<Q>(A, GC + lane / Q, lane % Q)] = w;
+                if constexpr (C::DATAFLOW) {
+                    __threadfence_block();
+                    __syncwarp();
+                    if (lane == 0) *(volatile int *)(s.bulkd + A) = D0;
+                }
                 if (tr) t_early += clock64() - tt0;
             }
         }
-        __syncthreads();
+        if constexpr (!C::DATAFLOW) __syncthreads();
         if (tr) { tb0 = clock64(); t_a += tb0 - ta0; }
         if (lp > 0) {
             for (int ie = warp; ie < nE; ie += C::NWARP) {
