@@ -76,8 +76,9 @@ extern "C" {
 #define RNA4R_TABLE_INT32  2
 
 /* ---- fill engines ---- */
-#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 10, else DIAG; rna4r_fold_batch takes SMEM when
-                                     4 <= q <= 8 and every sequence is <= rna4r_smem_max_n(ctx)  */
+#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 10, else DIAG; for 4 <= q <= 8 rna4r_fold_batch folds
+                                     the sequences of at most rna4r_smem_max_n(ctx) bases on SMEM and the
+                                     longer ones of the same batch on TILED                             */
 #define RNA4R_ENGINE_TILED  1     /* persistent super-tile wavefront, R resident in shared memory
                                      (the B200 design)                     */
 #define RNA4R_ENGINE_DIAG   2     /* paper-literal section 4 algorithm: one launch per anti-

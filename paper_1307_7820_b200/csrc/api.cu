@@ -94,7 +94,8 @@ int single_enqueue(rna4r_ctx *ctx, const uint8_t *seq_dev, const int64_t *offset
 size_t engine_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_single)
 {
     if (ctx->engine == RNA4R_ENGINE_SMEM) return smemseq::workspace_bytes(count);
-    if (ctx->engine == RNA4R_ENGINE_TILED) return tiled_ws(ctx, lens, count, n_single);
+    if (ctx->engine == RNA4R_ENGINE_TILED)      // AUTO may split a batch: the tiled engine's area, then the SMEM engine's
+        return align_up(tiled_ws(ctx, lens, count, n_single), 256) + (ctx->engine_auto ? smemseq::workspace_bytes(count) : 0);
     // per-sequence engines: sequences of a batch are folded one after another, each in its own slice
     size_t total = 0;
     for (int t = 0; t < count; ++t) total += single_ws(ctx, lens ? lens[t] : n_single);
@@ -154,7 +155,7 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0; ctx->max_blocks_per_sm = 0; ctx->max_blocks = 0;
     ctx->timing = 0; ctx->timing_valid = 0; ctx->ev0 = ctx->ev1 = nullptr;
     ctx->trace = nullptr; ctx->trace_tiles = 0;
-    ctx->engine_auto = 1; ctx->order_host = nullptr; ctx->order_cap = 0;
+    ctx->engine_auto = 1; ctx->order_host = nullptr; ctx->order_cap = 0; ctx->route_host = nullptr; ctx->route_cap = 0;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t N = (size_t)1 << q, M = (size_t)1 << (q - 1);
     auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4); delete ctx; return RNA4R_ERR_CUDA; };
@@ -189,6 +190,7 @@ int rna4r_destroy(rna4r_ctx *ctx)
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete[] ctx->order_host;
+    delete[] ctx->route_host;
     ctx->magic = 0;
     delete ctx;
     return RNA4R_OK;
@@ -300,7 +302,7 @@ size_t rna4r_workspace_bytes(const rna4r_ctx *ctx, int n_max, int count, int fla
     size_t core = 256;
     if (count > 0) {
         // every sequence at n_max: per-sequence cost is monotone in n
-        if (ctx->engine == RNA4R_ENGINE_TILED) core = (size_t)count * tiled_ws(ctx, nullptr, 1, n_max);
+        if (ctx->engine == RNA4R_ENGINE_TILED) core = (size_t)count * tiled_ws(ctx, nullptr, 1, n_max) + smemseq::workspace_bytes(count);
         else if (ctx->engine == RNA4R_ENGINE_SMEM) core = smemseq::workspace_bytes(count);
         else core = (size_t)count * single_ws(ctx, n_max);
     }
@@ -389,19 +391,45 @@ int rna4r_fold_batch_status(rna4r_ctx *ctx, const uint8_t *seqs_dev, const int64
         ctx->last_launches = launches;
         return RNA4R_OK;
     }
-    // Batches of short sequences go to the CTA-per-sequence engine when the engine was left on AUTO:
-    // every sequence's state has to fit one CTA's shared memory; otherwise the whole batch runs on the tiled engine.
-    bool use_smem = ctx->engine == RNA4R_ENGINE_SMEM;
-    if (!use_smem && ctx->engine_auto && smem_q_ok(ctx->q)) {
-        const int lim = smem_max_n(ctx->q);
-        use_smem = true;
-        for (int t = 0; t < count; ++t) if (lens_host[t] > lim) { use_smem = false; break; }
-    }
-    if (use_smem)
+    // AUTO: sequences whose state fits one CTA's shared memory go to the CTA-per-sequence engine, the
+    // longer ones of the same batch to the tiled engine (indexed through a map: nothing is copied or reordered).
+    if (ctx->engine == RNA4R_ENGINE_SMEM)
         return dispatch_q_smem(ctx->q, [&](auto Q) {
             return smemseq::enqueue_q<decltype(Q)::value>(ctx, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
                                                           status_out_dev, nullptr, RNA4R_TABLE_NONE, workspace_dev, st);
         });
+    if (ctx->engine_auto && smem_q_ok(ctx->q)) {
+        const int lim = smem_max_n(ctx->q);
+        int n_long = 0;
+        for (int t = 0; t < count; ++t) n_long += lens_host[t] > lim;
+        if (n_long < count) {
+            const size_t smem_off = n_long ? align_up(tiled_ws(ctx, lens_host, count, 0), 256) : 0;
+            int launches = 0;
+            if (n_long) {
+                if (count > ctx->route_cap) {
+                    int32_t *nb = new (std::nothrow) int32_t[2 * (size_t)count];
+                    if (!nb) return RNA4R_ERR_CUDA;
+                    delete[] ctx->route_host;
+                    ctx->route_host = nb; ctx->route_cap = count;
+                }
+                int32_t *idx = ctx->route_host, *len = idx + count;
+                for (int t = 0, k = 0; t < count; ++t) if (lens_host[t] > lim) { idx[k] = t; len[k++] = lens_host[t]; }
+                int rc = dispatch_q(ctx->q, [&](auto Q) {
+                    return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seqs_dev, offsets_dev, len, n_long, 0, scores_out_dev,
+                                                                status_out_dev, nullptr, RNA4R_TABLE_NONE, workspace_dev, st, idx);
+                });
+                if (rc != RNA4R_OK) return rc;
+                launches = ctx->last_launches;
+            }
+            int rc = dispatch_q_smem(ctx->q, [&](auto Q) {
+                return smemseq::enqueue_q<decltype(Q)::value>(ctx, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
+                                                              status_out_dev, nullptr, RNA4R_TABLE_NONE, (char *)workspace_dev + smem_off,
+                                                              st, true);
+            });
+            ctx->last_launches += launches;
+            return rc;
+        }
+    }
     return dispatch_q(ctx->q, [&](auto Q) {
         return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seqs_dev, offsets_dev, lens_host, count, 0, scores_out_dev,
                                                     status_out_dev, nullptr, RNA4R_TABLE_NONE, workspace_dev, st);

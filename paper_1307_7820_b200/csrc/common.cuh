@@ -27,6 +27,8 @@ struct rna4r_ctx {
     int engine_auto;         // the engine was left on (or set back to) RNA4R_ENGINE_AUTO: batches of short sequences take the SMEM engine
     int32_t *order_host;     // host scratch of the SMEM engine: sequence indices sorted by length (grown on demand)
     int order_cap;
+    int32_t *route_host;     // host scratch of a batch split between the SMEM and the tiled engine: indices | lengths of the long part
+    int route_cap;
 };
 // u64 words per super-tile in the optional trace buffer (rna4r_set_trace); a build with
 // -DRNA4R_TRACE_WORDS=256 adds per-q-tile event stamps for tuning

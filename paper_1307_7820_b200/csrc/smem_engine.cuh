@@ -620,14 +620,16 @@ static inline size_t workspace_bytes(int count) { return 256 + 2 * align_up((siz
 
 template <int Q>
 static int enqueue_q(rna4r_ctx *ctx, const uint8_t *seqs, const int64_t *offsets, const int32_t *lens_host, int count, int n_single,
-                     int32_t *scores, int32_t *status, void *table_out, int table_dtype, void *ws, cudaStream_t st)
+                     int32_t *scores, int32_t *status, void *table_out, int table_dtype, void *ws, cudaStream_t st,
+                     bool skip_long = false)
 {
+    // skip_long: sequences beyond max_n<Q>() belong to another engine's half of the batch and are left out
     using C = Cfg<Q>;
     Params p;
     p.seqs = seqs; p.offsets = offsets; p.lens = nullptr; p.order = nullptr; p.n_single = n_single;
     p.tbl = ctx->Rc; p.scores = scores; p.status = status; p.table_out = table_out; p.table_dtype = table_dtype;
     p.trace = ctx->trace; p.trace_seqs = ctx->trace_tiles;
-    int max_len = n_single;
+    int max_len = n_single, grid = count;
     if (offsets) {
         // longest first: the hardware hands CTAs to SMs in index order, so this is the LPT rule (work ~ n^3).
         // Counting sort by length into a context-owned host array (grown on demand, never per call).
@@ -637,14 +639,16 @@ static int enqueue_q(rna4r_ctx *ctx, const uint8_t *seqs, const int64_t *offsets
             delete[] ctx->order_host;
             ctx->order_host = nb; ctx->order_cap = count;
         }
+        const int lim = max_n<Q>();
         max_len = 0;
-        for (int t = 0; t < count; ++t) if (lens_host[t] > max_len) max_len = lens_host[t];
+        for (int t = 0; t < count; ++t) if (lens_host[t] > max_len && (!skip_long || lens_host[t] <= lim)) max_len = lens_host[t];
         {
             int hist[2050] = {0};
             if (max_len > 2048) return RNA4R_ERR_BAD_N;
-            for (int t = 0; t < count; ++t) ++hist[max_len - lens_host[t] + 1];
+            for (int t = 0; t < count; ++t) if (lens_host[t] <= max_len) ++hist[max_len - lens_host[t] + 1];
             for (int b = 1; b <= max_len + 1; ++b) hist[b] += hist[b - 1];
-            for (int t = 0; t < count; ++t) ctx->order_host[hist[max_len - lens_host[t]]++] = t;
+            grid = hist[max_len + 1];
+            for (int t = 0; t < count; ++t) if (lens_host[t] <= max_len) ctx->order_host[hist[max_len - lens_host[t]]++] = t;
         }
         char *base = (char *)ws;
         int32_t *lens_dev = (int32_t *)(base + 256);
@@ -659,10 +663,10 @@ static int enqueue_q(rna4r_ctx *ctx, const uint8_t *seqs, const int64_t *offsets
     auto kern = table_out ? seq_kernel<Q, true> : seq_kernel<Q, false>;
     RNA4R_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::MAX_SMEM));
     if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
-    kern<<<count, C::NTHR, smem, st>>>(p);
+    if (grid > 0) kern<<<grid, C::NTHR, smem, st>>>(p);
     if (ctx->timing) { RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev1, st)); ctx->timing_valid = 1; }
     RNA4R_CUDA(ctx, cudaGetLastError());
-    ctx->last_launches = 1;
+    ctx->last_launches = grid > 0 ? 1 : 0;
     return RNA4R_OK;
 }
 

@@ -136,6 +136,8 @@ struct Params {
     const uint8_t *seqs;
     const int64_t *offsets;   // device [count+1], or NULL for a single sequence of length n_single
     const int32_t *lens_dev;  // device copy of lens_host [count] (batch only): the geometry always follows the host plan
+    const int32_t *map;       // NULL, or device [count]: sequence t of this call is sequence map[t] of the caller's batch
+                              // (offsets, scores, status are indexed through it: a batch split between two engines)
     int32_t *status;          // NULL, or device [count]: RNA4R_STATUS_* bits per sequence
     int n_single;
     int count;
@@ -191,7 +193,8 @@ __global__ void plan_seq_kernel(Params p)
     if (threadIdx.x == 0) {
         SeqInfo si;
         si.n = n; si.nt = nt; si.pad[0] = si.pad[1] = si.pad[2] = 0;
-        si.invalid = (p.offsets && p.offsets[t + 1] - p.offsets[t] != (int64_t)n) ? RNA4R_STATUS_BAD_OFFSETS : 0;
+        const int o = p.map ? p.map[t] : t;
+        si.invalid = (p.offsets && p.offsets[o + 1] - p.offsets[o] != (int64_t)n) ? RNA4R_STATUS_BAD_OFFSETS : 0;
         si.sbase = atomicAdd(&p.hdr->ntiles, nt * (nt + 1) / 2);
         si.cbase = atomicAdd(&p.hdr->ncodes, nt * T);
         p.seqinfo[t] = si;
@@ -254,7 +257,7 @@ __global__ void encode_kernel(Params p)
         const SeqInfo si = p.seqinfo[t];
         const int len = si.nt * T;
         const bool readable = !(si.invalid & RNA4R_STATUS_BAD_OFFSETS);      // never read through offsets that failed the check
-        const uint8_t *src = p.seqs + (p.offsets && readable ? p.offsets[t] : 0);
+        const uint8_t *src = p.seqs + (p.offsets && readable ? p.offsets[p.map ? p.map[t] : t] : 0);
         bool bad = false;
         for (int x = blockIdx.x * blockDim.x + threadIdx.x; x < len; x += gridDim.x * blockDim.x) {
             int c = 4;
@@ -1286,8 +1289,9 @@ __device__ void run_close(const Params &p, const Smem<Q> &sm, const SeqInfo &si,
             }
         }
         if (I == 0 && J == n / T && tid == 0) {
-            p.scores[seq] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
-            if (p.status) p.status[seq] = si.invalid;
+            const int o = p.map ? p.map[seq] : seq;
+            p.scores[o] = si.invalid ? -1 : (int32_t)sm.val[(n - J * T) + 1];   // M(0,n) = D(1,n)
+            if (p.status) p.status[o] = si.invalid;
         }
         __syncthreads();               // orders every thread's stores before thread 0's releases (cumulative)
         if (tid == 0) {
@@ -1358,7 +1362,8 @@ static inline int pick_delta(int T, const int32_t *lens, int count, int n_single
 {
     int max_n = 0;
     for (int t = 0; t < count; ++t) { const int n = lens ? lens[t] : n_single; if (n > max_n) max_n = n; }
-    return (max_n / T + 1 > 128) ? 8 : 4;
+    const int nt = max_n / T + 1;
+    return nt > 192 ? 16 : nt > 128 ? 8 : 4;     // n = 16384: 18.0 ms with 8 and with 16, half the acc traffic with 16
 }
 
 struct HostPlan {
@@ -1384,7 +1389,7 @@ static inline HostPlan host_plan(int T, int delta, const int32_t *lens, int coun
 struct WsLayout {
     size_t zero_bytes;   // prefix that must be zeroed before every fold
     size_t off_hdr, off_stepC, off_stepP, off_curC, off_curP, off_done, off_accstage, off_rowprog, off_colprog;
-    size_t off_seqinfo, off_lens, off_tasks, off_codes, off_recs, off_acc, total;
+    size_t off_seqinfo, off_lens, off_map, off_tasks, off_codes, off_recs, off_acc, total;
 };
 
 static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int count)
@@ -1403,6 +1408,7 @@ static inline WsLayout ws_layout(int T, int rec_bytes, const HostPlan &h, int co
     w.off_seqinfo = off; off += align_up((size_t)count * sizeof(SeqInfo), 256);
     w.zero_bytes = off;
     w.off_lens = off; off += align_up((size_t)count * 4, 256);
+    w.off_map = off; off += align_up((size_t)count * 4, 256);
     w.off_tasks = off; off += align_up(h.tasks * sizeof(int4), 256);
     w.off_codes = off; off += align_up(h.codes, 256);
     w.off_recs = off; off += align_up(h.tiles * (size_t)rec_bytes, 256);
@@ -1423,7 +1429,7 @@ static size_t workspace_bytes_q(int delta, const int32_t *lens, int count, int n
 template <int Q>
 static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64_t *offsets, const int32_t *lens_host,
                      int count, int n_single, int32_t *scores, int32_t *status, void *table_out, int table_dtype, void *ws,
-                     cudaStream_t st)
+                     cudaStream_t st, const int32_t *map_host = nullptr)
 {
     using C = Cfg<Q>;
     if (delta <= 0) delta = pick_delta(C::T, lens_host, count, n_single);
@@ -1433,6 +1439,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     Params p;
     p.seqs = seqs; p.offsets = offsets; p.n_single = n_single; p.count = count; p.max_nt = h.max_nt; p.delta = delta;
     p.lens_dev = (const int32_t *)(base + w.off_lens); p.status = status;
+    p.map = map_host ? (const int32_t *)(base + w.off_map) : nullptr;
     p.hdr = (PlanHdr *)(base + w.off_hdr);
     p.stepC = (int *)(base + w.off_stepC); p.stepP = (int *)(base + w.off_stepP);
     p.curC = (int *)(base + w.off_curC); p.curP = (int *)(base + w.off_curP);
@@ -1460,6 +1467,8 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     RNA4R_CUDA(ctx, cudaMemsetAsync(ws, 0, w.zero_bytes, st));
     if (offsets)    // lens_host is consumed before this call returns (pageable memory is staged by the runtime)
         RNA4R_CUDA(ctx, cudaMemcpyAsync(base + w.off_lens, lens_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
+    if (map_host)
+        RNA4R_CUDA(ctx, cudaMemcpyAsync(base + w.off_map, map_host, (size_t)count * 4, cudaMemcpyHostToDevice, st));
     if (!offsets && h.max_nt <= 2048) {
         plan_single_kernel<Q><<<h.max_nt, 128, 0, st>>>(p); ++launches;          // plan + encode of a single fold: one launch
     } else {

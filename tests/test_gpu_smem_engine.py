@@ -166,17 +166,30 @@ def test_bad_offsets_status(rna):
     assert status.cpu().numpy().tolist() == [0, 2, 2]
 
 
-def test_auto_falls_back_to_tiled_for_long_sequences(rna):
-    """one sequence beyond the shared-memory limit: the whole batch runs on the tiled engine (more than one launch)"""
+def test_auto_splits_a_batch_between_the_engines(rna):
+    """sequences beyond the shared-memory limit run on the tiled engine (5 launches), the rest of the same batch on the
+    SMEM engine (1 launch); scores and status words land at the caller's indices; an all-long batch is all tiled"""
     r = ctx(rna, 8, rna.ENGINE_AUTO)
     rs = np.random.RandomState(7500)
     lim = r.smem_max_n()
-    seqs = [rand_seq(rs, n) for n in (100, lim + 1, 300)]
+    seqs = [rand_seq(rs, n) for n in (100, lim + 1, 300, 0, 1500, lim, 64)]
+    seqs[2] = seqs[2][:17] + b"X" + seqs[2][18:]
+    seqs[4] = seqs[4][:900] + b"n" + seqs[4][901:]
     flat, offsets, lens32 = workloads.pack_batch(seqs)
+    status = torch.full((len(seqs),), -7, dtype=torch.int32, device="cuda")
+    scores = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens32, status_out=status)
+    torch.cuda.synchronize()
+    assert r.last_launch_count() == 6
+    want = np.array([oracle.nussinov_fast(s)["score"] if len(s) > 400 else oracle.nussinov(s) for s in seqs])
+    assert want[2] == -1 and want[4] == -1
+    assert (scores.cpu().numpy() == want).all()
+    assert status.cpu().numpy().tolist() == [0, 0, 1, 0, 1, 0, 0]
+    longs = [seqs[1], seqs[4]]
+    flat, offsets, lens32 = workloads.pack_batch(longs)
     scores = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens32)
     torch.cuda.synchronize()
-    assert r.last_launch_count() > 1
-    assert (scores.cpu().numpy() == np.array([oracle.nussinov(s) for s in seqs])).all()
+    assert r.last_launch_count() == 5
+    assert scores.cpu().numpy().tolist() == [want[1], -1]
     rs_ = ctx(rna, 8, rna.ENGINE_SMEM)
     with pytest.raises(rna.Rna4rError) as e:
         rs_.fold(dev_seq(seqs[1]))

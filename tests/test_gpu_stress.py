@@ -38,7 +38,9 @@ def test_two_streams_back_to_back(rna):
     ra, rb = rna.Rna4r(8, 0, rna.ENGINE_TILED), rna.Rna4r(8, 0)
     sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
     fd, od, d3 = torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), dev(s3)
+    ra.set_engine(rna.ENGINE_AUTO)                 # the AUTO workspace also holds the SMEM engine's arrays
     wsa = torch.empty(ra.workspace_bytes_batch(lens32), dtype=torch.uint8, device="cuda")
+    ra.set_engine(rna.ENGINE_TILED)
     wsb = torch.empty(rb.workspace_bytes(len(s3)), dtype=torch.uint8, device="cuda")
     NA, NB = 200, 50
     outa = torch.full((NA, len(lens32)), -7, dtype=torch.int32, device="cuda")
