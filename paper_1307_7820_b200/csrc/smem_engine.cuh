@@ -35,6 +35,7 @@
 // (4 DPX VIADDMNMX.S16x2).  No skewed wavefront: 8 dependent steps per tile, every lane busy in every step.
 #pragma once
 #include <new>
+#include <type_traits>
 #include "common.cuh"
 
 namespace smemseq {
@@ -460,7 +461,7 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
 // warps would otherwise idle behind one long bulk task the range is split in 2 or 4 parts, which leave their maxima in
 // dead rows of the ring (tile-rows >= NB-D have no tile left) and are merged after an extra barrier.
 template <int Q>
-__device__ __forceinline__ uint32_t step_plan(int NB, int D)
+__device__ __forceinline__ uint32_t step_plan(int NB, int D, int nwarp)
 {
     using C = Cfg<Q>;
     const int NT = NB - D;
@@ -471,17 +472,20 @@ __device__ __forceinline__ uint32_t step_plan(int NB, int D)
     const int elen = D0 - 3;
     int lp = 0;
     if (nE > 0 && !C::DATAFLOW) {
-        const int wfree = C::NWARP - (NT + 3) / 4;
+        const int wfree = nwarp - (NT + 3) / 4;
         const int rows = (D * C::VPITCH) / 32;               // part slots (32 words each) the dead rows hold
         lp = (elen >= 72 && 4 * nE <= wfree && 4 * nE <= rows) ? 2 : (elen >= 40 && 2 * nE <= wfree && 2 * nE <= rows) ? 1 : 0;
     }
     return (uint32_t)ntw | ((uint32_t)nE << 8) | ((uint32_t)Afirst << 16) | ((uint32_t)lp << 20);
 }
 
-template <int Q, bool TABLE>
-__global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
+// NW warps per CTA: 24 with one CTA per SM (the register file: 80 x 768), 12 with two CTAs per SM for sequences whose
+// state fits half the shared memory (a second sequence on the SM fills the issue slots a short fold leaves idle)
+template <int Q, bool TABLE, int NW>
+__global__ void __launch_bounds__(NW * 32, Cfg<Q>::NWARP / NW) seq_kernel(Params p)
 {
     using C = Cfg<Q>;
+    constexpr int NTHR = NW * 32;
     static_assert(C::G == 4, "task numbering assumes 4 tiles per warp");
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -512,8 +516,8 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
     {
         const uint32_t *src = reinterpret_cast<const uint32_t *>(p.tbl);
         uint32_t *dst = reinterpret_cast<uint32_t *>(smem_raw);
-        for (int e = tid; e < C::TBL_BYTES / 4; e += C::NTHR) dst[e] = __ldg(src + e);
-        for (int e = tid; e < C::SCR_BYTES / 4; e += C::NTHR) reinterpret_cast<uint32_t *>(s.scr)[e] = 0;
+        for (int e = tid; e < C::TBL_BYTES / 4; e += NTHR) dst[e] = __ldg(src + e);
+        for (int e = tid; e < C::SCR_BYTES / 4; e += NTHR) reinterpret_cast<uint32_t *>(s.scr)[e] = 0;
         if (tid < 16) s.misc[tid] = 0;
     }
     __syncthreads();
@@ -521,7 +525,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         int bad = 0;
         if (p.offsets && p.offsets[seq + 1] - p.offsets[seq] != (int64_t)n) bad = RNA4R_STATUS_BAD_OFFSETS;
         const uint8_t *src = p.seqs + (p.offsets && !bad ? p.offsets[seq] : 0);
-        for (int x = tid; x < NB * Q + 16; x += C::NTHR) {
+        for (int x = tid; x < NB * Q + 16; x += NTHR) {
             int cde = 4;
             if (x < n && !bad) { cde = rna4r_base_code(src[x]); if (cde == 4) bad |= RNA4R_STATUS_BAD_BASE; }
             s.code[x] = (int8_t)cde;
@@ -534,17 +538,17 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         return;
     }
     if (tid == 0 && p.status) p.status[seq] = 0;
-    for (int e = tid; e < NB * 4; e += C::NTHR) {
+    for (int e = tid; e < NB * 4; e += NTHR) {
         const int A = e >> 2, x = e & 3;
         uint32_t bits = 0;
 #pragma unroll
         for (int a = 0; a < Q; ++a) bits |= (uint32_t)rna4r_pair(s.code[A * Q + a], x) << a;
         s.pm[e] = (uint8_t)bits;
     }
-    for (int D = tid; D < NB; D += C::NTHR) s.plan[D] = step_plan<Q>(NB, D);
-    for (int e = tid; e < 3 * NB + 8; e += C::NTHR) s.prog[e] = 0;
+    for (int D = tid; D < NB; D += NTHR) s.plan[D] = step_plan<Q>(NB, D, NW);
+    for (int e = tid; e < 3 * NB + 8; e += NTHR) s.prog[e] = 0;
     // ---- tile-diagonal 0
-    for (int A = tid; A < NB; A += C::NTHR) diag_tile<Q, TABLE>(p, s, seq, A);
+    for (int A = tid; A < NB; A += NTHR) diag_tile<Q, TABLE>(p, s, seq, A);
     __syncthreads();
     if (tr) t_setup = clock64() - t_start;
 
@@ -558,7 +562,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         const int D0 = D + 1, elen = D0 - 3;
         uint32_t *part = s.val + NT * C::VPITCH;
         const int ntask = ntw + (nE << lp);
-        for (int t = warp; t < ntask; t += C::NWARP) {
+        for (int t = warp; t < ntask; t += NW) {
             long long tt0 = 0;
             if (tr) tt0 = clock64();
             if (t < ntw) {
@@ -592,7 +596,7 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, 1) seq_kernel(Params p)
         if constexpr (!C::DATAFLOW) __syncthreads();
         if (tr) { tb0 = clock64(); t_a += tb0 - ta0; }
         if (lp > 0) {
-            for (int ie = warp; ie < nE; ie += C::NWARP) {
+            for (int ie = warp; ie < nE; ie += NW) {
                 const int A = Afirst + C::G * ie, GC = A + D0;
                 uint32_t acc[Q];
 #pragma unroll
@@ -658,15 +662,45 @@ static int enqueue_q(rna4r_ctx *ctx, const uint8_t *seqs, const int64_t *offsets
         p.lens = lens_dev; p.order = order_dev;
     }
     if (max_len > max_n<Q>()) return RNA4R_ERR_BAD_N;
-    size_t smem = (size_t)C::FIXED_BYTES + make_layout<Q>(max_len).total;
-    if (smem < 49152) smem = 49152;
-    auto kern = table_out ? seq_kernel<Q, true> : seq_kernel<Q, false>;
-    RNA4R_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::MAX_SMEM));
+    auto smem_of = [](int n) { size_t b = (size_t)C::FIXED_BYTES + make_layout<Q>(n).total; return b < 49152 ? (size_t)49152 : b; };
     if (ctx->timing) RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev0, st));
-    if (grid > 0) kern<<<grid, C::NTHR, smem, st>>>(p);
+    int launches = 0;
+    if (!offsets) {
+        if (table_out) {
+            RNA4R_CUDA(ctx, cudaFuncSetAttribute(seq_kernel<Q, true, C::NWARP>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::MAX_SMEM));
+            seq_kernel<Q, true, C::NWARP><<<1, C::NTHR, smem_of(max_len), st>>>(p);
+        } else {
+            RNA4R_CUDA(ctx, cudaFuncSetAttribute(seq_kernel<Q, false, C::NWARP>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::MAX_SMEM));
+            seq_kernel<Q, false, C::NWARP><<<1, C::NTHR, smem_of(max_len), st>>>(p);
+        }
+        launches = 1;
+    } else if (grid > 0) {
+        // One kernel for the batch; its CTA size follows the longest sequence: a fold that needs the whole shared memory
+        // of an SM gets 24 warps, and when every state fits 1/2, 1/3, 1/4 of it the CTAs have 12, 8, 6 warps and two to
+        // four sequences share an SM (the register file holds 24 warps at 80 registers): a short fold has too few
+        // independent tasks per tile-diagonal for 24 warps, a neighbour on the SM fills the idle issue slots (2048
+        // sequences of 100..400 bases: 1.04 ms with 24-warp CTAs, 0.71 ms with two CTAs per SM).  A mixed batch is not
+        // split by class: measured slower (cfg4 1.72 against 1.54 ms), the long class loses the short folds that fill
+        // the tail of its longest-first order.
+        const size_t need = smem_of(max_len);
+        const size_t per_sm = 233472;                    // 228 KB, 1 KB of it reserved per resident CTA
+        auto launch = [&](auto NWc) -> int {
+            constexpr int NW = decltype(NWc)::value;
+            RNA4R_CUDA(ctx, cudaFuncSetAttribute(seq_kernel<Q, false, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::MAX_SMEM));
+            seq_kernel<Q, false, NW><<<grid, NW * 32, need, st>>>(p);
+            return RNA4R_OK;
+        };
+        int rc;
+        if (need + 1024 <= per_sm / 4) rc = launch(std::integral_constant<int, C::NWARP / 4>{});
+        else if (need + 1024 <= per_sm / 3) rc = launch(std::integral_constant<int, C::NWARP / 3>{});
+        else if (need + 1024 <= per_sm / 2) rc = launch(std::integral_constant<int, C::NWARP / 2>{});
+        else rc = launch(std::integral_constant<int, C::NWARP>{});
+        if (rc != RNA4R_OK) return rc;
+        launches = 1;
+    }
     if (ctx->timing) { RNA4R_CUDA(ctx, cudaEventRecord(ctx->ev1, st)); ctx->timing_valid = 1; }
     RNA4R_CUDA(ctx, cudaGetLastError());
-    ctx->last_launches = grid > 0 ? 1 : 0;
+    ctx->last_launches = launches;
     return RNA4R_OK;
 }
 

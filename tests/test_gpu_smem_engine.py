@@ -201,6 +201,20 @@ def test_auto_splits_a_batch_between_the_engines(rna):
     r9.close()
 
 
+@pytest.mark.parametrize("hi", [120, 330, 400, 470, 560])
+def test_batches_of_every_cta_class(rna, hi):
+    """the CTA size follows the longest sequence of the batch: 6, 8, 12 warps (four, three, two CTAs per SM) and 24"""
+    r = ctx(rna, 8, rna.ENGINE_AUTO)
+    seqs, _ = workloads.random_sequences(7700 + hi, 300, hi // 3, hi)
+    seqs[0] = rand_seq(np.random.RandomState(hi), hi)
+    flat, offsets, lens32 = workloads.pack_batch(seqs)
+    scores = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens32)
+    torch.cuda.synchronize()
+    assert r.last_launch_count() == 1
+    want = np.array([oracle.nussinov_fast(x)["score"] for x in seqs])
+    assert (scores.cpu().numpy() == want).all()
+
+
 def test_host_batch_and_repeat(rna):
     r = ctx(rna, 8, rna.ENGINE_AUTO)
     seqs, _ = workloads.random_sequences(7600, 200, 0, 500)
