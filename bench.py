@@ -513,7 +513,7 @@ def also_workloads(pkg, torch, r8, flush):
     res["cfg4_batch1024_q8"] = {"ms": ms, "cell_k_updates_per_s": wtot / (ms * 1e-3), "fill_kernel_ms": r8.last_fill_kernel_ms(),
                                "lookups": ltot, "sum_scores": int(sc.sum().item()),
                                "engine": "smem (one CTA per sequence, one launch)" if r8.last_launch_count() == 1 else "tiled",
-                               "kernel": "smemseq::seq_kernel<8,false>" if r8.last_launch_count() == 1 else "tiled::fill_kernel<8>"}
+                               "kernel": "smemseq::seq_kernel<8,false,24>" if r8.last_launch_count() == 1 else "tiled::fill_kernel<8>"}
     # the same batch forced onto the long-sequence (tiled) engine: what the batch cost before the SMEM engine existed
     if r8.last_launch_count() == 1:
         rt = pkg.Rna4r(8, 0, pkg.ENGINE_TILED)

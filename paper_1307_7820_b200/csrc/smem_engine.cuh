@@ -345,6 +345,19 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
         while (!__all_sync(FULL, pg[A] >= D - 1 && pg[A + 1] >= D - 1 && (D0 < 4 || bd[A] >= D0))) __nanosleep(32);
         __threadfence_block();
     }
+    // Operands that do not depend on the fresh lookups are requested first: their shared-memory latency passes while
+    // the fresh loop runs (a single warp issues in order).  Bulk maxima of the strip-tile (written during step D0 - 1;
+    // none if the strip-tile starts before diagonal 4), the diagonal tile (B,B), the code of my column, the bottom edge
+    // M((A+1)q, c) = anchor of the column word of group A+1, and the left column M(r0+1+y, Bq-1) for lane 0's pair term:
+    // the last value tile (A,B-1) left in its rows, and for the row below the tile an anchor again.
+    uint32_t vw = 0;
+    if (D0 >= 4) vw = s.val[val_index<Q>(A, B, y)];
+    const uint2 qb = *reinterpret_cast<const uint2 *>(s.dq + (size_t)c * 8);
+    const int cc = s.code[c - 1];
+    int vprev = (int)(xcol[(A + 1) * Q] & C::XAMASK);
+    int Lc;
+    if (y < Q - 1) Lc = s.rl[r0 + 1 + y];
+    else Lc = (D >= 2) ? (int)(s.X[off_x<Q>(B - 1) + (A + 1) * Q + Q - 1] & C::XAMASK) : 0;
     // ---- fresh groups (a4): j in [0, min(k, D-2)] (column words of the tiles just below) and from max(D0-2, k+1) to
     // D-2 (row words of the tiles to the left inside the strip); without bulk (D0 < 4) that is every complete group
     uint32_t facc[Q];
@@ -364,34 +377,22 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
             j = (j == j1) ? j2 : j + 1;
         }
     }
-    // bulk maxima of the strip-tile, written during step D0 - 1 (none if the strip-tile starts before diagonal 4)
-    uint32_t vw = 0;
-    if (D0 >= 4) vw = s.val[val_index<Q>(A, B, y)];
+    // everything the rows below contribute without the wave: bulk and fresh maxima folded once
+#pragma unroll
+    for (int a = 0; a < Q; ++a) facc[a] = max(facc[a] & 0xffffu, (uint32_t)unpack_row<Q>(vw, a));
     // diagonal tile (B,B) for the tail: packed pairs (Qd(2j,y), Qd(2j+1,y)); y' > y is "minus infinity"
     int Qp[C::NP];
-    {
-        const uint2 qb = *reinterpret_cast<const uint2 *>(s.dq + (size_t)c * 8);
 #pragma unroll
-        for (int jj = 0; jj < C::NP; ++jj) {
-            const uint32_t src = jj < 2 ? qb.x : qb.y;
-            uint32_t pr = __byte_perm(src, 0, (jj & 1) ? 0x4342 : 0x4140);
-            if (2 * jj > y) pr |= 0x8000u;
-            if (2 * jj + 1 > y) pr |= 0x80000000u;
-            Qp[jj] = (int)pr;
-        }
+    for (int jj = 0; jj < C::NP; ++jj) {
+        const uint32_t src = jj < 2 ? qb.x : qb.y;
+        uint32_t pr = __byte_perm(src, 0, (jj & 1) ? 0x4342 : 0x4140);
+        if (2 * jj > y) pr |= 0x8000u;
+        if (2 * jj + 1 > y) pr |= 0x80000000u;
+        Qp[jj] = (int)pr;
     }
     // pairing mask of my column against the rows of the tile-row: bit a <-> b(S[r0+a], S[c-1])
     uint32_t pm = 0;
-    {
-        const int cc = s.code[c - 1];
-        if (cc < 4) pm = s.pm[A * 4 + cc];
-    }
-    // bottom edge M((A+1)q, c): anchor of the column word of group A+1; left column M(r0+1+y, Bq-1) for lane 0's
-    // pair term: the last value tile (A,B-1) left in its rows, and for the row below the tile an anchor again
-    int vprev = (int)(xcol[(A + 1) * Q] & C::XAMASK);
-    int Lc;
-    if (y < Q - 1) Lc = s.rl[r0 + 1 + y];
-    else Lc = (D >= 2) ? (int)(s.X[off_x<Q>(B - 1) + (A + 1) * Q + Q - 1] & C::XAMASK) : 0;
+    if (cc < 4) pm = s.pm[A * 4 + cc];
     const uint32_t *wh = s.wdh + r0;
     uint16_t *scr = s.scr + (size_t)warp * C::SCR_WARP_HW;
     // lanes that own no output store to a per-warp dummy word instead of predicating every store
@@ -407,10 +408,8 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
         // ---- candidates from the rows below: bulk, fresh, pair term (a3), head residual (a5)
         const int lca = __shfl_sync(FULL, Lc, i * Q + a);
         const int vd = (y == 0) ? lca : vl;
-        int cand = unpack_row<Q>(vw, a);
-        cand = max(cand, vd + (int)((pm >> a) & 1u));
-        uint32_t best = lookup_max<Q>(s.tbl_sa, wh[a] + Xp, (uint32_t)cand);
-        best = __vmaxu2(best, facc[a]);
+        const int cand = max((int)facc[a], vd + (int)((pm >> a) & 1u));
+        const uint32_t best = lookup_max<Q>(s.tbl_sa, wh[a] + Xp, (uint32_t)cand);
         // ---- tail: V(a,y) = max_{y' <= y} C'(a,y') + Qd(y',y)
         uint16_t *row = rowbase + (a & 1) * (C::G * 8);
         if (lane_ok) row[y] = (uint16_t)(best & 0xffffu);
