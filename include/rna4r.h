@@ -23,8 +23,12 @@
  *     (sequence, outputs, workspace) and the stream.  The library allocates only what
  *     rna4r_prepare creates (the R tables) and frees it in rna4r_destroy.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
- *   - rna4r_fold / rna4r_fold_batch only ENQUEUE work on `stream` and return; they never
- *     allocate and never synchronise.  The *_host variants copy in/out and synchronise `stream`.
+ *   - rna4r_fold / rna4r_fold_batch only ENQUEUE work on `stream` and return; they never allocate
+ *     device memory and never synchronise.  (rna4r_fold_batch keeps two small context-owned HOST
+ *     index arrays -- the batch sorted by length, the sequences routed to the tiled engine -- which
+ *     grow when a batch holds more sequences than any before.)  The *_host variants copy in/out and
+ *     synchronise `stream`.
+ *   - A workspace size is valid for the engine setting it was asked with (rna4r_set_engine).
  *   - Every function returns 0 (RNA4R_OK) or a negative RNA4R_ERR_* code; nothing throws.
  *   - There is NO CPU fallback: on a machine without an sm_100 device rna4r_prepare fails with
  *     RNA4R_ERR_DEVICE and nothing else can be called.
