@@ -215,6 +215,21 @@ def test_batches_of_every_cta_class(rna, hi):
     assert (scores.cpu().numpy() == want).all()
 
 
+@pytest.mark.parametrize("q", [5, 8])
+def test_random_batches_over_the_whole_length_range(rna, q):
+    """lengths anywhere in 0..smem_max_n, mixed in one batch (the 24-warp class), several batches"""
+    r = ctx(rna, q, rna.ENGINE_AUTO)
+    lim = r.smem_max_n()
+    for rep in range(3):
+        seqs, _ = workloads.random_sequences(7800 + 10 * q + rep, 150, 0, lim)
+        flat, offsets, lens32 = workloads.pack_batch(seqs)
+        scores = r.fold_batch(torch.from_numpy(flat).cuda(), torch.from_numpy(offsets).cuda(), lens32)
+        torch.cuda.synchronize()
+        assert r.last_launch_count() == 1
+        want = np.array([oracle.nussinov_fast(x, threads=2)["score"] for x in seqs])
+        assert (scores.cpu().numpy() == want).all(), (q, rep)
+
+
 def test_host_batch_and_repeat(rna):
     r = ctx(rna, 8, rna.ENGINE_AUTO)
     seqs, _ = workloads.random_sequences(7600, 200, 0, 500)
