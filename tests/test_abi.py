@@ -39,6 +39,20 @@ def test_header_compiles_as_c_and_a_c_program_calls_the_abi(tmp_path):
     assert "c_abi_check ok" in out.stdout
 
 
+def test_smem_engine_layout_fits_config4(tmp_path):
+    """the SMEM engine's shared-memory plan (host logic): config 4's longest sequence fits, regions aligned and disjoint"""
+    import shutil
+    import subprocess
+    if shutil.which("nvcc") is None:
+        pytest.skip("nvcc not on PATH")
+    exe = str(tmp_path / "smem_layout_check")
+    subprocess.check_call(["nvcc", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe,
+                           os.path.join(ROOT, "tests", "smem_layout_check.cu")])
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0, (out.returncode, out.stdout)
+    assert "smem_layout_check ok" in out.stdout and "q=8 max_n=70" in out.stdout
+
+
 def test_strerror_and_version_need_no_gpu():
     from paper_1307_7820_b200 import load
     L = load()
