@@ -80,11 +80,12 @@ extern "C" {
 #define RNA4R_TABLE_INT32  2
 
 /* ---- fill engines ---- */
-#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 10, else DIAG; for 4 <= q <= 8 rna4r_fold_batch folds
+#define RNA4R_ENGINE_AUTO   0     /* TILED when 2 <= q <= 11, else DIAG; for 4 <= q <= 8 rna4r_fold_batch folds
                                      the sequences of at most rna4r_smem_max_n(ctx) bases on SMEM and the
                                      longer ones of the same batch on TILED                             */
 #define RNA4R_ENGINE_TILED  1     /* persistent super-tile wavefront, R resident in shared memory
-                                     (the B200 design)                     */
+                                     (the B200 design); q in 2..11 (q = 9..11
+                                     index the table in base 3, see rna4r_table_to_host)        */
 #define RNA4R_ENGINE_DIAG   2     /* paper-literal section 4 algorithm: one launch per anti-
                                      diagonal, one thread per cell, per-cell sliding vectors
                                      (PAPER.md:249-267); any q in 2..12; the comparison point   */
@@ -128,8 +129,12 @@ const uint8_t *rna4r_table(const rna4r_ctx *ctx);
 /* Device pointer to the compact table Rc (uint8[2^(q-1)][2^(q-1)]), or NULL. */
 const uint8_t *rna4r_table_compact(const rna4r_ctx *ctx);
 
-/* Copies R (compact = 0: 2^q * 2^q bytes) or Rc (compact = 1: 2^(q-1) * 2^(q-1) bytes) into HOST memory
- * dst_host after synchronising the device (a test / inspection helper).  Errors: CONTEXT, NULL, CUDA. */
+/* Copies R (compact = 0: 2^q * 2^q bytes), Rc (compact = 1: 2^(q-1) * 2^(q-1) bytes) or the ternary-indexed
+ * form Rt (compact = 2: 3^(q-1) bytes; exists for q = 9, 10 and 11 only, otherwise RNA4R_ERR_ENGINE) into HOST
+ * memory dst_host after synchronising the device (a test / inspection helper).  The black box
+ * adds v_k and vbar_k in every step, so max-val depends on the pair only through d_k = v_k + vbar_k in
+ * {-1, 0, 1}:  Rt[sum_{k=1}^{q-1} (d_k + 1) 3^(k-1)] = R[v][vbar] with bit k of v = v_k, bit k of vbar = |vbar_k|.
+ * Errors: CONTEXT, NULL, BAD_N (compact not 0..2), ENGINE, CUDA. */
 int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact);
 
 /* Selects the fill engine (RNA4R_ENGINE_*) for later fold calls.  Errors: CONTEXT, ENGINE. */
@@ -268,7 +273,7 @@ int rna4r_trace_to_host(rna4r_ctx *ctx, uint64_t *dst_host, int tiles);
  * as the fill kernel issues it, and times it with CUDA events on `stream` (synchronises):
  *   variant 0 (context q = 8):  add, address, 1-byte shared-memory gather, add-max; operands in registers;
  *   variant 1 (context q = 8):  the bulk product's inner loop (operand words loaded from shared memory);
- *   variant 2 (context q = 10): the nibble-table sequence; operands in registers.
+ *   variant 2 (context q = 10): variant 0 on the ternary-indexed table of 3^9 entries; operands in registers.
  *   iters           loop trips per thread, 1..16000 (16 lookups per trip; variant 1: 128 per trip).
  *   blocks_per_sm   CTAs of 256 threads per SM (0 = as many as fit).
  *   workspace_dev   device scratch, >= 256 bytes.

@@ -138,6 +138,12 @@ class Rna4r:
     def table_compact(self) -> np.ndarray:
         return self._table_host(1)
 
+    def table_ternary(self) -> np.ndarray:
+        """Rt, 3^(q-1) bytes indexed by sum (v_k + vbar_k + 1) 3^(k-1); q = 9..11 only (rna4r.h)."""
+        out = np.empty(3 ** (self.q - 1), dtype=np.uint8)
+        _check(self.lib.rna4r_table_to_host(self.h, out.ctypes.data, 2), "rna4r_table_to_host")
+        return out
+
     def _table_host(self, compact: int) -> np.ndarray:
         side = 1 << (self.q - 1 if compact else self.q)
         out = np.empty((side, side), dtype=np.uint8)

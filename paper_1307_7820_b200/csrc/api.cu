@@ -40,18 +40,17 @@ auto dispatch_q(int q, F &&f) -> decltype(f(std::integral_constant<int, 8>{}))
     case 7: return f(std::integral_constant<int, 7>{});
     case 8: return f(std::integral_constant<int, 8>{});
     case 9: return f(std::integral_constant<int, 9>{});
-    default: return f(std::integral_constant<int, 10>{});
+    case 10: return f(std::integral_constant<int, 10>{});
+    default: return f(std::integral_constant<int, 11>{});
     }
 }
 
-// largest n the tagged 32-bit words of the tiled engine can hold: anchor sums + q < 2^(32-SH)
+// largest n the tagged 32-bit words of the tiled engine can hold: the value field is 16 bits for every q
+// (tiled::Cfg: ISHIFT = 16), anchor sums + q < 2^16 with D <= n/2, so the ABI's limit n <= 65534 (int16 table) is the only one
 inline int tiled_max_n(int q)
 {
-    const int sh = 2 * (q - 1);
-    const long long lim = (1ll << (32 - sh)) - 1 - q;   // max value of A + B + rv
-    long long n = 2 * lim;                              // D <= n/2
-    if (n > 65534) n = 65534;
-    return (int)n;
+    (void)q;
+    return 65534;
 }
 
 size_t tiled_ws(const rna4r_ctx *ctx, const int32_t *lens, int count, int n_single)
@@ -149,21 +148,23 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
     rna4r_ctx *ctx = new (std::nothrow) rna4r_ctx();
     if (!ctx) return RNA4R_ERR_CUDA;
     ctx->magic = RNA4R_MAGIC; ctx->q = q; ctx->device = device;
-    ctx->engine = (q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
+    ctx->engine = (q <= 11) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
     ctx->sm_count = prop.multiProcessorCount;
-    ctx->R = ctx->Rc = ctx->Rc4 = nullptr;
+    ctx->R = ctx->Rc = ctx->Rt = nullptr;
     ctx->last_launches = 0; ctx->last_cuda_error = 0; ctx->tiled_blocks_per_sm = 0; ctx->max_blocks_per_sm = 0; ctx->max_blocks = 0;
     ctx->timing = 0; ctx->timing_valid = 0; ctx->ev0 = ctx->ev1 = nullptr;
     ctx->trace = nullptr; ctx->trace_tiles = 0;
     ctx->engine_auto = 1; ctx->order_host = nullptr; ctx->order_cap = 0; ctx->route_host = nullptr; ctx->route_cap = 0;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t N = (size_t)1 << q, M = (size_t)1 << (q - 1);
-    auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4); delete ctx; return RNA4R_ERR_CUDA; };
+    auto fail = [&](cudaError_t e) { ctx->last_cuda_error = (int)e; cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rt); delete ctx; return RNA4R_ERR_CUDA; };
     cudaError_t e;
     if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&ctx->R, N * N)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&ctx->Rc, M * M < 16 ? 16 : M * M)) != cudaSuccess) return fail(e);
-    if ((e = cudaMalloc(&ctx->Rc4, M * M / 2 < 16 ? 16 : M * M / 2)) != cudaSuccess) return fail(e);
+    uint32_t tern = 0;                                   // 3^(q-1) entries, built for the q that use them (tiled::Cfg::TERN)
+    if (q >= RNA4R_TERN_MIN_Q && q <= 11) { tern = 1; for (int k = 1; k < q; ++k) tern *= 3u; }
+    if (tern && (e = cudaMalloc(&ctx->Rt, (tern + 15u) & ~15u)) != cudaSuccess) return fail(e);
     {
         const size_t total = N * N;
         const int cap = ctx->sm_count * 16;
@@ -172,9 +173,13 @@ int rna4r_prepare(int q, int device, void *stream, rna4r_ctx **out)
         const size_t tc = M * M;
         blocks = (int)((tc + 255) / 256); if (blocks > cap) blocks = cap;
         rna4r_build_compact_kernel<<<blocks, 256, 0, st>>>(q, ctx->R, ctx->Rc);
-        rna4r_pack_nibbles_kernel<<<blocks, 256, 0, st>>>(tc, ctx->Rc, ctx->Rc4);
+        ctx->last_launches = 2;
+        if (tern) {
+            if ((e = cudaMemsetAsync(ctx->Rt, 0, (tern + 15u) & ~15u, st)) != cudaSuccess) return fail(e);
+            rna4r_build_ternary_kernel<<<(int)((tern + 255u) / 256u), 256, 0, st>>>(q, tern, ctx->Rt);
+            ctx->last_launches = 3;
+        }
         if ((e = cudaGetLastError()) != cudaSuccess) return fail(e);
-        ctx->last_launches = 3;
     }
     *out = ctx;
     return RNA4R_OK;
@@ -185,7 +190,7 @@ int rna4r_destroy(rna4r_ctx *ctx)
     if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rc4);
+    cudaFree(ctx->R); cudaFree(ctx->Rc); cudaFree(ctx->Rt);
     cudaFree(ctx->trace);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
@@ -210,6 +215,14 @@ int rna4r_table_to_host(rna4r_ctx *ctx, uint8_t *dst_host, int compact)
     if (!dst_host) return RNA4R_ERR_NULL;
     RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
     RNA4R_CUDA(ctx, cudaDeviceSynchronize());
+    if (compact < 0 || compact > 2) return RNA4R_ERR_BAD_N;
+    if (compact == 2) {                                  // the ternary-indexed table, 3^(q-1) bytes (q = 9..11 only)
+        if (!ctx->Rt) return RNA4R_ERR_ENGINE;
+        size_t entries = 1;
+        for (int k = 1; k < ctx->q; ++k) entries *= 3;
+        RNA4R_CUDA(ctx, cudaMemcpy(dst_host, ctx->Rt, entries, cudaMemcpyDeviceToHost));
+        return RNA4R_OK;
+    }
     const size_t side = (size_t)1 << (compact ? ctx->q - 1 : ctx->q);
     RNA4R_CUDA(ctx, cudaMemcpy(dst_host, compact ? ctx->Rc : ctx->R, side * side, cudaMemcpyDeviceToHost));
     return RNA4R_OK;
@@ -268,9 +281,9 @@ int rna4r_set_engine(rna4r_ctx *ctx, int engine)
 {
     if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
     const int is_auto = engine == RNA4R_ENGINE_AUTO;
-    if (is_auto) engine = (ctx->q <= 10) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
+    if (is_auto) engine = (ctx->q <= 11) ? RNA4R_ENGINE_TILED : RNA4R_ENGINE_DIAG;
     if (engine != RNA4R_ENGINE_TILED && engine != RNA4R_ENGINE_SMEM && !per_sequence_engine(engine)) return RNA4R_ERR_ENGINE;
-    if (engine == RNA4R_ENGINE_TILED && ctx->q > 10) return RNA4R_ERR_ENGINE;
+    if (engine == RNA4R_ENGINE_TILED && ctx->q > 11) return RNA4R_ERR_ENGINE;
     if (engine == RNA4R_ENGINE_SMEM && !smem_q_ok(ctx->q)) return RNA4R_ERR_ENGINE;
     ctx->engine = engine;
     ctx->engine_auto = is_auto;

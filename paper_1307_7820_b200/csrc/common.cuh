@@ -13,7 +13,7 @@ struct rna4r_ctx {
     int sm_count;
     uint8_t *R;              // device uint8[2^q][2^q]
     uint8_t *Rc;             // device uint8[2^(q-1)][2^(q-1)]   reachable quadrant, Rc[h][w] = R[2h][2w]
-    uint8_t *Rc4;            // device nibble-packed Rc (two entries per byte), only when 2(q-1) > 16
+    uint8_t *Rt;             // device ternary-indexed table, 3^(q-1) entries (rtable.cuh), q = 9..11 only (else NULL)
     int last_launches;
     int last_cuda_error;
     int tiled_blocks_per_sm; // occupancy of the tiled fill kernel for this q (0 = not queried yet)

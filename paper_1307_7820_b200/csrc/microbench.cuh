@@ -10,7 +10,7 @@
 //   variant 0  "pure":    operands in registers, 16 independent lookups per loop trip (the instruction floor);
 //   variant 1  "product": tiled::product_accumulate as the bulk product runs it (row words by broadcast LDS.128,
 //                         column words per lane, 16 lookups per 2 + 2 operand loads) on a resident panel pair;
-//   variant 2  "nibble":  the q = 10 sequence (mask, word load, nibble extract, shifted add, max), operands in registers.
+//   variant 2  "ternary": variant 0 on the q = 10 table of 3^9 entries (same four instructions), operands in registers.
 #pragma once
 #include "tiled_engine.cuh"
 
@@ -25,10 +25,10 @@ __device__ __forceinline__ void stage_table(const Smem<Q> &sm, const uint8_t *tb
 {
     using C = Cfg<Q>;
     constexpr int ROWB = 1 << C::HB;
-    if constexpr (C::NIBBLE) {
+    if constexpr (C::TERN) {
         const uint4 *src = reinterpret_cast<const uint4 *>(tbl);
         uint4 *dst = reinterpret_cast<uint4 *>(sm.tbl);
-        for (int e = tid; e < C::TBL_BYTES / 16; e += nthr) dst[e] = __ldg(src + e);
+        for (int e = tid; e < (C::TBL_BYTES + 15) / 16; e += nthr) dst[e] = __ldg(src + e);
     } else {
         for (int e = tid; e < ROWB * ROWB; e += nthr) sm.tbl[(e / ROWB) * C::TBL_PITCH + e % ROWB] = tbl[e];
     }
@@ -96,7 +96,7 @@ static int run(rna4r_ctx *ctx, int iters, int blocks_per_sm, uint32_t *sink, cud
     cudaEvent_t e0, e1;
     RNA4R_CUDA(ctx, cudaEventCreate(&e0));
     RNA4R_CUDA(ctx, cudaEventCreate(&e1));
-    const uint8_t *tbl = C::NIBBLE ? ctx->Rc4 : ctx->Rc;
+    const uint8_t *tbl = C::TERN ? ctx->Rt : ctx->Rc;
     lookup_kernel<Q, VARIANT><<<blocks, 256, C::SMEM_BYTES, st>>>(tbl, iters / 8 + 1, sink);     // warm-up
     cudaEventRecord(e0, st);
     lookup_kernel<Q, VARIANT><<<blocks, 256, C::SMEM_BYTES, st>>>(tbl, iters, sink);

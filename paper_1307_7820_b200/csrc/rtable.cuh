@@ -35,10 +35,20 @@ __global__ void rna4r_build_compact_kernel(int q, const uint8_t *__restrict__ R,
     }
 }
 
-// Nibble packing of Rc for q where the byte table no longer fits shared memory (q = 10: 2^18
-// entries, values 0..9 -> 128 KB).  Entry e lives in byte e/2, low nibble for even e.
-__global__ void rna4r_pack_nibbles_kernel(size_t entries, const uint8_t *__restrict__ Rc, uint8_t *__restrict__ Rc4)
+// Ternary form of the same table for q >= 10, where 2^(2(q-1)) bytes no longer fit shared memory.  The listing
+// PAPER.md:94-111 adds v_k and vbar_k in every step, so its result depends on the two vectors only through
+// d_k = v_k - |vbar_k| in {-1, 0, 1}:  Rt[sum_{k=1}^{q-1} (d_k + 1) 3^(k-1)] = max(0, max_k sum_{k'<=k} d_k'),
+// 3^(q-1) entries (19 683 at q = 10).  Entry (h, w) of Rc is Rt[sum_k (h_k + 1 - w_k) 3^(k-1)].
+__global__ void rna4r_build_ternary_kernel(int q, uint32_t entries, uint8_t *__restrict__ Rt)
 {
-    for (size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x; b < entries / 2; b += (size_t)gridDim.x * blockDim.x)
-        Rc4[b] = (uint8_t)((Rc[2 * b] & 15) | ((Rc[2 * b + 1] & 15) << 4));
+    for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < entries; e += gridDim.x * blockDim.x) {
+        uint32_t x = e;
+        int maxval = 0, sum = 0;                            // line 1-2; k = 0 adds v_0 + vbar_0 = 0
+        for (int k = 1; k < q; ++k) {                       // line 3
+            sum += (int)(x % 3u) - 1;                       // line 4-5: v_k + vbar_k
+            x /= 3u;
+            if (sum > maxval) maxval = sum;                 // line 6-7
+        }
+        Rt[e] = (uint8_t)maxval;
+    }
 }

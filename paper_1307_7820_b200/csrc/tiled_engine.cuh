@@ -14,11 +14,10 @@
 // Each (row, group) is one 32-bit word W = anchor M(r,gq) + index bits h, and each (group, column) one word
 // X = anchor M(gq,c) + index bits v  (HB = q-1 bits each, SH = 2*HB index bits, h above v).  Then S = W + X
 // carries the table index and the anchor sum in disjoint fields, and the candidate is S + Rc[idx] on the value
-// field.  Two layouts (Cfg::F16): q <= 9 keeps the value in the low halfword and the index in the high one, so
+// field.  The value sits in the low halfword and the index in the high one (binary for q <= 9, ternary above), so
 // that the gather address is (S >> 16) + base (one LEA.HI) and "max(acc, S + rv)" is one DPX instruction
-// (VIADDMNMX.U16x2) -- add, address, LDS.U8, add-max; q = 10 (18 index bits) keeps the index in the low SH bits
-// and the value above them (S + (rv << SH), unsigned max).  The index bits left in a candidate are harmless:
-// they never change the order of the value field.
+// (VIADDMNMX.U16x2) -- add, address, LDS.U8, add-max.  The index bits left in a candidate are harmless: they never
+// change the order of the value field.  q >= 10 indexes a table of 3^(q-1) entries in base 3 (Cfg::TERN).
 //
 // Decomposition.  Super-tiles of T = 8q cells (8 groups) per side.  For super-tile (I,J), I < J:
 //   * every group lying in a block K strictly between I and J is a "full group" for ALL T*T cells
@@ -34,6 +33,10 @@
 #pragma once
 #include "common.cuh"
 
+#ifndef RNA4R_TERN_MIN_Q
+#define RNA4R_TERN_MIN_Q 9        // smallest q that indexes the table in base 3 (Cfg::TERN)
+#endif
+
 namespace tiled {
 
 
@@ -44,28 +47,41 @@ struct Cfg {
     static constexpr int HB = Q - 1;           // informative bits per vector
     static constexpr int SH = 2 * HB;          // table index bits
     static constexpr uint32_t IDXMASK = (1u << SH) - 1u;
-    // Word format.  F16 (q <= 9): value in bits [0,16), table index in bits [16,16+SH): a candidate is
+    // Word format (F16, every q): value in bits [0,16), table index in bits [16,32): a candidate is
     // max(acc, S + rv) on the low halfword -- ONE DPX instruction (VIADDMNMX.U16x2; the high halfword carries
-    // harmless index bits), and the gather address is (S >> 16) + base -- one LEA.HI.  q = 10 needs 18 index
-    // bits: index in bits [0,SH), value above (S + (rv << SH), plain unsigned max).
-    static constexpr bool F16 = (SH <= 16);
-    static constexpr int VSHIFT = F16 ? 0 : SH;      // position of the value field
-    static constexpr int ISHIFT = F16 ? 16 : 0;      // position of the index field
-    static constexpr bool NIBBLE = (SH > 16);  // q = 10: nibble-packed table (128 KB)
-    // F16: the table rows (2^HB bytes, one per h) are stored with a pitch of 2^HB + 4 bytes.  A row of 128 bytes
-    // covers the 32 banks exactly once, so with the natural pitch the bank of a gather depends on v alone and the
-    // closure's gathers -- different h per lane, partial (mostly zero) v -- pile up on a few banks (ncu: 7-way
-    // conflicts).  With the padded pitch the bank is (h + v/4) mod 32; the bulk product (one h per warp) stays
-    // conflict-free.  The index field of a row word is then h * TBL_PITCH (a sum of per-bit constants), not a
-    // bit field; the column word still adds v.
-    static constexpr int TBL_PITCH = (F16 && Q <= 8) ? (1 << HB) + 4 : (1 << HB);     // q = 9: 256 x 260 would overflow the halfword
-    static constexpr int TBL_BYTES = NIBBLE ? (1 << SH) / 2 : (1 << HB) * TBL_PITCH;
-    static constexpr uint32_t VMASK = ((1u << HB) - 1u) << ISHIFT;      // the v bits of a column word
+    // harmless index bits), and the gather address is (S >> 16) + base -- one LEA.HI.
+    //
+    // q <= 8: BINARY index h * pitch + v.  The table rows (2^HB bytes, one per h) are stored with a
+    // pitch of 2^HB + 4 bytes.  A row of 128 bytes covers the 32 banks exactly once, so with the natural
+    // pitch the bank of a gather depends on v alone and the closure's gathers -- different h per lane, partial (mostly
+    // zero) v -- pile up on a few banks (ncu: 7-way conflicts).  With the padded pitch the bank is (h + v/4) mod 32; the
+    // bulk product (one h per warp) stays conflict-free.  The index field of a row word is then h * TBL_PITCH (a sum
+    // of per-bit constants), not a bit field; the column word still adds v.
+    //
+    // q >= 9 (RNA4R_TERN_MIN_Q): TERNARY index.  The black box sees the two vectors only through d_k = v_k - |vbar_k| in
+    // {-1,0,1}: R[h][v] = max(0, max_k sum_{k'<=k} d_k').  A table indexed by sum_k (h_k + 1 - v_k) 3^k has 3^(q-1)
+    // entries (6 561 bytes at q = 9, 19 683 at q = 10, 59 049 at q = 11, against 2^16, 2^18 and 2^20), and the index is still the sum of a
+    // row part sum h_k 3^k and a column part sum (1 - v_k) 3^k -- base-3 digits 0..2, no carries -- so S = W + X and
+    // the four-instruction lookup stay as they are.  The price: the gathers of a warp scatter over the whole table
+    // (bank conflicts, as a binary table wider than 128 bytes per row has them too), where the layout of q <= 8 has
+    // none in the bulk product.  Measured on cfg5 (n = 16384): q = 9 37.3 -> 27.1 ms, q = 10 (nibble-packed binary
+    // table before) 41.7 -> 23.6 ms, q = 11 25.5 ms (not possible before).
+    static constexpr bool TERN = (Q >= RNA4R_TERN_MIN_Q);
+    static constexpr bool F16 = true;
+    static constexpr int VSHIFT = 0;           // position of the value field
+    static constexpr int ISHIFT = 16;          // position of the index field
+    __host__ __device__ static constexpr uint32_t pow3(int k) { return k <= 0 ? 1u : 3u * pow3(k - 1); }
+    static constexpr uint32_t TERN_C0 = (pow3(HB) - 1u) / 2u;      // index part of a column word without set bits: sum_k 3^k
+    static_assert(TERN ? pow3(HB) <= 65536u : SH <= 16, "the table index has to fit the high halfword");
+    static constexpr int TBL_PITCH = TERN ? 1 : (Q <= 8 ? (1 << HB) + 4 : (1 << HB));     // q = 9: 256 x 260 would overflow the halfword
+    static constexpr int TBL_BYTES = TERN ? (int)pow3(HB) : (1 << HB) * TBL_PITCH;
+    static constexpr uint32_t VMASK = ((1u << HB) - 1u) << ISHIFT;      // the v bits of a (binary) column word
     static constexpr int TBL_AREA = (TBL_BYTES + 15) / 16 * 16;
     static constexpr int PTHR = 4 * T;         // threads that take part in a bulk product (T columns x 4 row blocks)
     static constexpr int WTHR = PTHR > 256 ? PTHR : 256;   // product threads, and at least the 8 closure warps
     static constexpr int NTHR = WTHR + 128;    // + 4 warps: a closure needs NROLE = NWV + NMH + 8 warps
-    static constexpr int MIN_CTAS = (Q <= 8) ? 3 : 1;   // register budget: 3 CTAs per SM while the table is small
+    static constexpr int MIN_CTAS = (Q <= 8) ? 3 : ((TERN && Q <= 10) ? 2 : 1);   // register budget: 3 CTAs per SM with the byte table of q <= 8,
+                                               // 2 with the ternary tables of q = 9, 10 (q = 9 at 3 CTAs: 48 registers, spills, 3 % faster on cfg5 -- not taken)
     static constexpr int RPT = Q;              // product phase: a thread owns RPT rows x 2 columns (c and c + T/2): the warp-uniform
     static constexpr int HT = T / 2;           // row words are loaded once for 2*RPT lookups (a broadcast LDS.128 costs 2 wavefronts)
     static constexpr int TP = T + 8;           // pitch of the per-group word arrays (bank spread)
@@ -364,37 +380,26 @@ struct Smem {
 };
 
 // One table gather (the unit of work of this path): rv = Rc[index field of S].  SAFE marks the call sites where
-// S may be a don't-care value of an idle lane (q = 10 masks the index anyway; F16 relies on the window size).
+// S may be a don't-care value of an idle lane (the window is at least 64 KB + 16 long: any 16-bit index stays inside).
 template <int Q, bool SAFE = false>
 __device__ __forceinline__ uint32_t tbl_gather(const Smem<Q> &sm, uint32_t S)
 {
-    using C = Cfg<Q>;
-    if constexpr (C::NIBBLE) {
-        const uint32_t idx = S & C::IDXMASK;
-        const uint32_t w = reinterpret_cast<const uint32_t *>(sm.tbl)[idx >> 3];
-        return (w >> ((idx & 7u) * 4u)) & 15u;
-    } else if constexpr (C::F16) {
-        const uint32_t idx = S >> 16;                 // no mask: see Cfg::SMEM_BYTES
-        uint32_t rv;
-        asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"(idx + sm.tbl_sa));
-        return rv;
-    } else {
-        return sm.tbl[S & C::IDXMASK];
-    }
+    const uint32_t idx = S >> 16;                 // no mask: see Cfg::SMEM_BYTES
+    uint32_t rv;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(rv) : "r"(idx + sm.tbl_sa));
+    return rv;
 }
 
 // tagged values: (value << VSHIFT) | don't-care bits of the index field
 template <int Q> __device__ __forceinline__ uint32_t tag_value(int v) { return (uint32_t)v << Cfg<Q>::VSHIFT; }
-template <int Q> __device__ __forceinline__ int untag(uint32_t x) { return Cfg<Q>::F16 ? (int)(x & 0xffffu) : (int)(x >> Cfg<Q>::SH); }
-template <int Q> __device__ __forceinline__ uint32_t tag_max(uint32_t a, uint32_t b) { return Cfg<Q>::F16 ? __vmaxu2(a, b) : max(a, b); }
+template <int Q> __device__ __forceinline__ int untag(uint32_t x) { return (int)(x & 0xffffu); }
+template <int Q> __device__ __forceinline__ uint32_t tag_max(uint32_t a, uint32_t b) { return __vmaxu2(a, b); }
 
 // acc = max(acc, candidate of the word sum S): eq. (3)
 template <int Q, bool SAFE = false>
 __device__ __forceinline__ uint32_t lookup_max(const Smem<Q> &sm, uint32_t S, uint32_t acc)
 {
-    const uint32_t rv = tbl_gather<Q, SAFE>(sm, S);
-    if constexpr (Cfg<Q>::F16) return __viaddmax_u16x2(S, rv, acc);
-    else return max(acc, S + (rv << Cfg<Q>::SH));
+    return __viaddmax_u16x2(S, tbl_gather<Q, SAFE>(sm, S), acc);
 }
 
 // Polls are relaxed loads (an acquire load also invalidates the L1 on every iteration); one acquire load
@@ -684,7 +689,7 @@ template <int Q, bool DIAG, bool MERGED>
 __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int lane, bool own)
 {
     using C = Cfg<Q>;
-    constexpr int TP = C::TP, VP = C::VP, SH = C::SH;
+    constexpr int TP = C::TP, VP = C::VP;
     constexpr uint32_t FULL = 0xffffffffu;
     constexpr int ZOFF = DIAG ? 0 : 8;
     const int y = lane % Q;                              // lane group lane/Q runs q-tile (A,B); !own: shadow, stores nothing
@@ -693,7 +698,13 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
     const uint32_t w2mask = (y >= 2) ? FULL : 0u;
     const int c = B * Q + y;
     const int abot = A * Q + Q - 1;
-    const uint32_t khy = ((uint32_t)C::TBL_PITCH << (y > 0 ? y - 1 : 0)) << C::ISHIFT;   // index weight of my horizontal difference bit
+    uint32_t khy = ((uint32_t)C::TBL_PITCH << (y > 0 ? y - 1 : 0)) << C::ISHIFT;   // index weight of my horizontal difference bit
+    if constexpr (C::TERN) {                             // 3^(y-1) instead of 2^(y-1)
+        khy = 1u << C::ISHIFT;
+#pragma unroll
+        for (int k = 1; k < Q - 1; ++k) if (k < y) khy *= 3u;
+    }
+    uint32_t w3 = 0;                                     // TERN: index weight 3^(Q-1-x) of the next vertical difference bit
     const int sh0 = C::ISHIFT + Q - 2 + y;                  // vertical bit of row x = s-y sits at sh0 - (s-1) (sh0 <= 31)
     const uint32_t XJ = MERGED ? 0u : sm.Xst[(ZOFF + B) * TP + c];
     uint32_t pms = 0;                                    // bit (x + y) <-> row x pairs with my column
@@ -740,8 +751,8 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         // depend on the shuffle result and cannot be scheduled -- with their wait for the gathers -- before the
         // shuffles are issued (a single warp issues in order).
         uint32_t best = tag_value<Q>(max(max(o_pend, vprev), Lv));
-        if (!MERGED) best = Cfg<Q>::F16 ? __viaddmax_u16x2(phS, phR, best) : max(best, phS + (phR << SH));
-        best = Cfg<Q>::F16 ? __viaddmax_u16x2(ptS, ptR, best) : max(best, ptS + (ptR << SH));
+        if (!MERGED) best = __viaddmax_u16x2(phS, phR, best);
+        best = __viaddmax_u16x2(ptS, ptR, best);
         int v = untag<Q>(best);
         if (s + 1 < Q && y == s + 1) v = vbelow;                    // pre-step (x = -1): the cell below the q-tile
         if (MERGED && s - (Q - 1) <= 1) v = 0;                      // D(i,i) = D(i,i-1) = 0
@@ -762,8 +773,16 @@ __device__ __forceinline__ void qtile_wave(const Smem<Q> &sm, int A, int B, int 
         o_pend = max(o_cur, Lv + (int)((pms >> ((s + 1) & 31)) & 1u));
         // ---- step a6, vertical: the column word now starts at row a (anchor v, bit of the pair (a, a+1))
         {
-            const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 1 ? s - 1 : 0) & 31);   // used for x >= 1 only
-            xbits = (y <= s - 1) ? ((xbits | dbit) & C::VMASK) : 0u;     // x >= 1
+            if constexpr (C::TERN) {
+                // a column word without set bits has the index part sum_k 3^k (digit 1 = "no difference"); the bit of
+                // the pair (row x, row x-1) takes 3^(Q-1-x) away.  The weight goes down by a factor 3 per row (an exact
+                // division; beyond the top row of the q-tile it runs out, those lanes are not live).
+                if (y <= s - 1) { xbits -= (uint32_t)(v - vprev) * w3; w3 = __umulhi(w3, 0xAAAAAAABu) >> 1; }
+                else { xbits = C::TERN_C0 << C::ISHIFT; w3 = C::pow3(Q - 2) << C::ISHIFT; }
+            } else {
+                const uint32_t dbit = ((uint32_t)(v - vprev) << sh0) >> ((s >= 1 ? s - 1 : 0) & 31);   // used for x >= 1 only
+                xbits = (y <= s - 1) ? ((xbits | dbit) & C::VMASK) : 0u;     // x >= 1
+            }
             vsh = vnew;
         }
         if (x_lo >= 0 && live && y == x_lo) sm.Xst[A * TP + c] = xbits + vsh;    // x = Q-1: the column word is complete
@@ -1315,8 +1334,8 @@ __global__ void __launch_bounds__(Cfg<Q>::NTHR, Cfg<Q>::MIN_CTAS) fill_kernel(Pa
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(p.tbl);
         uint4 *dst = reinterpret_cast<uint4 *>(sm.tbl);
-        if constexpr (C::TBL_PITCH == (1 << C::HB)) {
-            for (int e = tid; e < C::TBL_BYTES / 16; e += C::NTHR) dst[e] = __ldg(src + e);
+        if constexpr (C::TERN || C::TBL_PITCH == (1 << C::HB)) {
+            for (int e = tid; e < (C::TBL_BYTES + 15) / 16; e += C::NTHR) dst[e] = __ldg(src + e);       // the device tables are padded to 16 bytes
             if (C::TBL_BYTES < 16) for (int e = tid; e < C::TBL_BYTES; e += C::NTHR) sm.tbl[e] = p.tbl[e];
         } else {
             // padded pitch: row h of the compact table -> byte offset h * TBL_PITCH
@@ -1450,7 +1469,7 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     p.codes = (int8_t *)(base + w.off_codes);
     p.recs = (uint8_t *)(base + w.off_recs);
     p.acc = (int16_t *)(base + w.off_acc);
-    p.tbl = C::NIBBLE ? ctx->Rc4 : ctx->Rc;
+    p.tbl = C::TERN ? ctx->Rt : ctx->Rc;
     p.scores = scores; p.table_out = table_out; p.table_dtype = table_dtype;
     p.trace = ctx->trace; p.trace_tiles = ctx->trace_tiles;
     p.sm_count = ctx->sm_count;

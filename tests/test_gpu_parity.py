@@ -59,6 +59,31 @@ def test_rtable_entry_by_entry(rna, q):
     r.close()
 
 
+@pytest.mark.parametrize("q", [9, 10, 11])
+def test_ternary_rtable_entry_by_entry(rna, q):
+    """Rt[sum_k (v_k - |vbar_k| + 1) 3^(k-1)] == R[v][vbar] for every pair of vectors with bit 0 clear (rna4r.h);
+    the pairs reach every one of the 3^(q-1) entries"""
+    r = rna.Rna4r(q, 0)
+    Rt = r.table_ternary()
+    want = oracle.rtable(q)[::2, ::2]
+    M = 1 << (q - 1)
+    h = np.arange(M, dtype=np.int64)[:, None]
+    w = np.arange(M, dtype=np.int64)[None, :]
+    idx = np.zeros((M, M), dtype=np.int64)
+    for k in range(q - 1):
+        idx += (((h >> k) & 1) - ((w >> k) & 1) + 1) * 3 ** k
+    assert Rt.shape == (3 ** (q - 1),)
+    assert (Rt[idx] == want).all()
+    assert np.unique(idx).size == Rt.size
+    r.close()
+    with pytest.raises(rna.Rna4rError):
+        r8 = rna.Rna4r(8, 0)
+        try:
+            r8.table_ternary()
+        finally:
+            r8.close()
+
+
 # ------------------------------------------------------------------ full-table parity, small n
 ENGINES = ["tiled", "diag", "paper_tile", "maxplus"]
 
@@ -69,9 +94,11 @@ def engine_id(pkg, name):
 
 
 @pytest.mark.parametrize("engine", ENGINES)
-@pytest.mark.parametrize("q", list(range(2, 11)))
+@pytest.mark.parametrize("q", list(range(2, 13)))
 def test_full_table_all_small_n(rna, engine, q):
     """every n in 0..3q+2 (all residues mod q, n < q, n = 0,1,2) -- SURVEY section 4 tier (iv)"""
+    if engine == "tiled" and q > 11:
+        pytest.skip("the tiled engine stops at q = 11 (3^11 table bytes do not fit shared memory)")
     r = ctx(rna, q, engine_id(rna, engine))
     rs = np.random.RandomState(1000 + q)
     for n in range(0, 3 * q + 3):
@@ -88,7 +115,7 @@ def test_full_table_all_small_n(rna, engine, q):
 
 
 @pytest.mark.parametrize("engine", ENGINES)
-@pytest.mark.parametrize("q", [2, 3, 4, 5, 7, 8, 9, 10])
+@pytest.mark.parametrize("q", [2, 3, 4, 5, 7, 8, 9, 10, 11])
 def test_full_table_tile_boundaries_and_random(rna, engine, q):
     """lengths around the super-tile size T = 8q (ragged tails, several tiles) and random lengths"""
     r = ctx(rna, q, engine_id(rna, engine))
@@ -213,7 +240,7 @@ def test_cfg3_n6000_q8_comparison_engines(rna, engine):
     check_large(rna, "cfg3", 8, engine_id(rna, engine))
 
 
-@pytest.mark.parametrize("q", [8, 10])
+@pytest.mark.parametrize("q", [8, 10, 11])
 def test_cfg5_n16384(rna, q):
     check_large(rna, "cfg5", q, rna.ENGINE_TILED)
 
@@ -222,6 +249,13 @@ def test_cfg6_n32768_q8(rna):
     """beyond the five configs: n = 32768, score-only call, then the 2 GB int16 table against the
     oracle's stored cells, table sum and Lemma 1"""
     check_large(rna, "cfg6", 8, rna.ENGINE_TILED)
+
+
+@pytest.mark.parametrize("q", [10, 11])
+def test_cfg6_n32768_ternary_q(rna, q):
+    """n = 32768 at the q that index the table in base 3 (a 16-bit value field: anchor sums up to n/2 + q fit; the
+    binary 18-bit index of q = 10 stopped at n = 32746): the same stored cells, table sum and Lemma 1"""
+    check_large(rna, "cfg6", q, rna.ENGINE_TILED)
 
 
 def test_cfg4_batch_1024(rna):
@@ -303,7 +337,7 @@ def test_determinism_repeat_calls(rna):
 
 
 # ------------------------------------------------------------------ pipelined closures, late products, q sweep
-@pytest.mark.parametrize("q", [5, 8, 9, 10])
+@pytest.mark.parametrize("q", [5, 8, 9, 10, 11])
 def test_midsize_scores_every_late_product_shape(rna, q):
     """lengths of 2..9 super-tiles per side: super-tile diagonals dp = 1 (no late product), 2 (one block, both
     operands arriving), 3 (two late blocks, no bulk stage) and >= 4 (bulk stages + late blocks); sampled cells
@@ -336,7 +370,7 @@ def test_skewed_base_distributions(rna):
         assert got_score == want_score and (got.astype(np.int32) == want).all(), p
 
 
-@pytest.mark.parametrize("q", [4, 9, 10])
+@pytest.mark.parametrize("q", [4, 9, 10, 11])
 def test_batch_other_q(rna, q):
     r = ctx(rna, q, rna.ENGINE_TILED)
     seqs, _ = workloads.random_sequences(500 + q, 40, 0, 450)
@@ -347,9 +381,9 @@ def test_batch_other_q(rna, q):
 
 
 def test_length_limit_of_the_word_format(rna):
-    """q = 10 keeps 14 value bits above its 18 index bits: n <= 2 * (2^14 - 1 - q); q <= 9 takes the ABI's 65534"""
+    """every q keeps a 16-bit value field below the index field (q >= 9: base-3 index): the ABI's n <= 65534 holds"""
     r10 = ctx(rna, 10, rna.ENGINE_TILED)
-    lim = 2 * ((1 << 14) - 1 - 10)
+    lim = 65534
     assert r10.workspace_bytes(lim) > 0
     with pytest.raises(rna.Rna4rError) as e:
         r10.fold(dev_seq(b"A" * 16), n=lim + 1, workspace=torch.empty(1 << 20, dtype=torch.uint8, device="cuda"))

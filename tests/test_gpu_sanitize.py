@@ -14,7 +14,7 @@ torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("q", [4, 8, 10])
+@pytest.mark.parametrize("q", [4, 8, 10, 11])
 def test_small_folds_and_one_batch(q):
     if not torch.cuda.is_available():
         pytest.fail("needs a CUDA device (no CPU fallback exists)")

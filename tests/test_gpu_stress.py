@@ -73,7 +73,7 @@ def test_two_streams_back_to_back(rna):
     rb.close()
 
 
-@pytest.mark.parametrize("q", [4, 8, 10])
+@pytest.mark.parametrize("q", [4, 8, 10, 11])
 def test_every_grid_size(rna, q):
     """the task list is claimed in order and a claimed task only waits on earlier ones: any grid completes and
     gives the same table -- 1, 2, 3, 7 CTAs in all, then 1..3 CTAs per SM"""
