@@ -486,7 +486,7 @@ def also_workloads(pkg, torch, r8, flush):
     del tab3
     # q sweep at n = 6000 (the paper saw the serial gains saturate at q = 8-9)
     sweep = {}
-    for q in (4, 5, 6, 7, 8, 9, 10):
+    for q in (4, 5, 6, 7, 8, 9, 10, 11):
         rq = r8 if q == 8 else pkg.Rna4r(q, 0)
         sweep[str(q)] = time_call(lambda: rq.fold(d3), 5)
         if q != 8:
@@ -537,12 +537,14 @@ def also_workloads(pkg, torch, r8, flush):
     # cfg5
     s = workloads.single_config("cfg5")
     d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()
-    for q in (8, 10):
-        rr = r8 if q == 8 else pkg.Rna4r(10, 0)
+    for q in (8, 10, 11):                      # q = 10 is BASELINE.json's second cfg5 point; q = 11 the last q of the tiled engine
+        rr = r8 if q == 8 else pkg.Rna4r(q, 0)
         rr.enable_kernel_timing(True)
         ms = time_call(lambda: rr.fold(d), 3)
         res[f"cfg5_n16384_q{q}"] = {"ms": ms, "cell_k_updates_per_s": nussinov_updates(len(s)) / (ms * 1e-3),
                                     "fill_kernel_ms": rr.last_fill_kernel_ms(), "lookups": algorithmic_lookups(len(s), q)}
+        if q != 8:
+            rr.close()
     # cfg6: n = 32768 (beyond BASELINE.json's configs), score only
     s = workloads.single_config("cfg6")
     d = torch.from_numpy(np.frombuffer(s, dtype=np.uint8).copy()).cuda()
