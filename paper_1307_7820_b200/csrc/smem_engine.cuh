@@ -71,6 +71,12 @@ struct Cfg {
     // instead of the CTA barrier per tile-diagonal.  Measured equal (cfg4 1.60 vs 1.59 ms): the barrier is not what a
     // sequence waits for, the chain of waves through its neighbours is.
     static constexpr bool DATAFLOW = RNA4R_SMEM_DATAFLOW != 0;
+#ifndef RNA4R_SMEM_TOPUP
+#define RNA4R_SMEM_TOPUP 1
+#endif
+    // top-up tasks: the groups a strip-tile's bulk pass had to leave out for its later tile columns (they were not
+    // finished yet) are looked up one step before the tile closes, off the wave's path; the wave keeps two fresh groups
+    static constexpr bool TOPUP = !DATAFLOW && RNA4R_SMEM_TOPUP != 0;
     static constexpr int MAX_SMEM = 232448;          // 227 KB
 };
 
@@ -364,7 +370,9 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
 #pragma unroll
     for (int a = 0; a < Q; ++a) facc[a] = 0;
     {
-        const int j1 = min(k, D - 2), j2 = max(D0 - 2, k + 1);
+        // with top-up tasks only the two groups that were finished in the previous step are left: j = 0 and j = D-2
+        const bool topped = C::TOPUP && D0 >= 4;
+        const int j1 = topped ? 0 : min(k, D - 2), j2 = topped ? D - 2 : max(D0 - 2, k + 1);
         const int nf = (j1 + 1) + max(D - 1 - j2, 0);
         int j = 0;
 #pragma unroll 1
@@ -455,8 +463,54 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
     }
 }
 
+// ---- top-up: for the tiles that close in the NEXT step (tile-diagonal D1) and sit in column k >= 1 of their strip-tile,
+// the groups the strip-tile's bulk pass could not take and that are finished by now -- j in [1, k] (column words of the
+// tiles below, closed up to step D1-2) and [max(D0-2, k+1), D1-3] (row words of the tiles to the left) -- are merged into
+// the packed bulk word.  Same lane layout and task numbering as the wave; u counts the tasks with k != 0.
+template <int Q>
+__device__ __forceinline__ void topup_task(const Sm<Q> &s, int D1, int u, int lane)
+{
+    using C = Cfg<Q>;
+    const int NB = s.NB, NT = NB - D1;
+    const int skip = (4 - (D1 & 3)) & 3;                       // the residue of A with k = (A + D1) mod 4 = 0
+    const int r = u % 3, rho = r + (r >= skip ? 1 : 0);
+    const int A0 = rho + 16 * (u / 3);
+    if (A0 >= NT) return;
+    const bool lane_ok = lane < C::SW;
+    const int i = lane_ok ? lane / Q : C::G - 1;
+    const int y = lane_ok ? lane - i * Q : Q - 1;
+    int A = A0 + C::G * i;
+    const bool own = lane_ok && A < NT;
+    if (A >= NT) A = A0;
+    const int B = A + D1;
+    const int k = B & (C::G - 1), D0 = D1 - k;
+    if (D0 < 4) return;                                        // no bulk word yet: the wave looks everything up (warp-uniform)
+    const uint16_t *xcol = s.X + off_x<Q>(B) + y;
+    const uint32_t *wrow = s.W + off_w<Q>(NB, A);
+    uint32_t *slot = s.val + val_index<Q>(A, B, y);
+    const uint32_t vw = *slot;
+    uint32_t facc[Q];
+#pragma unroll
+    for (int a = 0; a < Q; ++a) facc[a] = 0;
+    const int j1 = min(k, D1 - 3), j2 = max(D0 - 2, k + 1);
+    const int nf = j1 + max(D1 - 2 - j2, 0);
+    int j = 1;
+#pragma unroll 1
+    for (int f = 0; f < nf; ++f) {
+        const uint32_t X32 = expand_x<Q>(xcol[(A + 1 + j) * Q]);
+        uint32_t wr[Q];
+        load_rows<Q>(wrow + j * Q, wr);
+#pragma unroll
+        for (int a = 0; a < Q; ++a) facc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, facc[a]);
+        j = (j == j1) ? j2 : j + 1;
+    }
+#pragma unroll
+    for (int a = 0; a < Q; ++a) facc[a] = max(facc[a] & 0xffffu, (uint32_t)unpack_row<Q>(vw, a));
+    if (own) *slot = pack_rows<Q>(facc);
+}
+
 // Plan of tile-diagonal step D: ntw wave tasks | nE bulk tasks << 8 | first tile-row of a bulk task << 16 | log2(parts)
-// << 20.  Bulk tasks: the strip-tiles (A, GC = A + D0) that start on diagonal D0 = D+1 >= 4, groups j in [1, D0-3]; when
+// << 20 (2 bits) | top-up tasks << 24.  Bulk tasks: the strip-tiles (A, GC = A + D0) that start on diagonal D0 = D+1 >= 4, groups j in [1, D0-3]; when
 // warps would otherwise idle behind one long bulk task the range is split in 2 or 4 parts, which leave their maxima in
 // dead rows of the ring (tile-rows >= NB-D have no tile left) and are merged after an extra barrier.
 template <int Q>
@@ -470,12 +524,14 @@ __device__ __forceinline__ uint32_t step_plan(int NB, int D, int nwarp)
     const int nE = (D0 >= 4 && D0 < NB && NB - 1 - D0 >= Afirst) ? ((NB - 1 - D0 - Afirst) >> 2) + 1 : 0;
     const int elen = D0 - 3;
     int lp = 0;
+    // top-up tasks for the tiles of diagonal D+1: three of the four residues of A (k != 0)
+    const int ntu = (C::TOPUP && D + 1 < NB && D + 1 >= 5) ? 3 * ((NT - 1 + 15) >> 4) : 0;
     if (nE > 0 && !C::DATAFLOW) {
-        const int wfree = nwarp - (NT + 3) / 4;
+        const int wfree = nwarp - (NT + 3) / 4 - ntu;
         const int rows = (D * C::VPITCH) / 32;               // part slots (32 words each) the dead rows hold
         lp = (elen >= 72 && 4 * nE <= wfree && 4 * nE <= rows) ? 2 : (elen >= 40 && 2 * nE <= wfree && 2 * nE <= rows) ? 1 : 0;
     }
-    return (uint32_t)ntw | ((uint32_t)nE << 8) | ((uint32_t)Afirst << 16) | ((uint32_t)lp << 20);
+    return (uint32_t)ntw | ((uint32_t)nE << 8) | ((uint32_t)Afirst << 16) | ((uint32_t)lp << 20) | ((uint32_t)ntu << 24);
 }
 
 // NW warps per CTA: 24 with one CTA per SM (the register file: 80 x 768), 12 with two CTAs per SM for sequences whose
@@ -557,16 +613,21 @@ __global__ void __launch_bounds__(NW * 32, Cfg<Q>::NWARP / NW) seq_kernel(Params
         const int NT = NB - D;
         // Tasks of the step (step_plan), dealt round-robin to the warps, waves first
         const uint32_t plan = s.plan[D];
-        const int ntw = (int)(plan & 0xffu), nE = (int)((plan >> 8) & 0xffu), Afirst = (int)((plan >> 16) & 3u), lp = (int)(plan >> 20);
+        const int ntw = (int)(plan & 0xffu), nE = (int)((plan >> 8) & 0xffu), Afirst = (int)((plan >> 16) & 3u), lp = (int)((plan >> 20) & 3u);
+        const int ntu = (int)(plan >> 24);
         const int D0 = D + 1, elen = D0 - 3;
         uint32_t *part = s.val + NT * C::VPITCH;
-        const int ntask = ntw + (nE << lp);
+        const int nbulk = nE << lp;
+        const int ntask = ntw + nbulk + ntu;                       // dealt in this order: waves, bulk, top-ups
         for (int t = warp; t < ntask; t += NW) {
             long long tt0 = 0;
             if (tr) tt0 = clock64();
             if (t < ntw) {
                 wave_task<Q, TABLE>(p, s, seq, D, t, warp, lane);
                 if (tr) { t_wave += clock64() - tt0; ++n_wave; }
+            } else if (t >= ntw + nbulk) {
+                topup_task<Q>(s, D + 1, t - ntw - nbulk, lane);
+                if (tr) t_early += clock64() - tt0;
             } else {
                 const int e = t - ntw, ie = e >> lp, pe = e & ((1 << lp) - 1);
                 const int A = Afirst + C::G * ie, GC = A + D0;
