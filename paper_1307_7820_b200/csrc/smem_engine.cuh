@@ -373,16 +373,26 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
         // with top-up tasks only the two groups that were finished in the previous step are left: j = 0 and j = D-2
         const bool topped = C::TOPUP && D0 >= 4;
         const int j1 = topped ? 0 : min(k, D - 2), j2 = topped ? D - 2 : max(D0 - 2, k + 1);
-        const int nf = (j1 + 1) + max(D - 1 - j2, 0);
-        int j = 0;
-#pragma unroll 1
-        for (int f = 0; f < nf; ++f) {
-            const uint32_t X32 = expand_x<Q>(xcol[(A + 1 + j) * Q]);
-            uint32_t wr[Q];
-            load_rows<Q>(wrow + j * Q, wr);
+        if (topped) {
+            // two groups (D >= 4 here), written side by side: one round of operand loads, two independent gathers per row
+            const uint32_t Xa = expand_x<Q>(xcol[(A + 1) * Q]), Xb = expand_x<Q>(xcol[(A + 1 + j2) * Q]);
+            uint32_t wa[Q], wb[Q];
+            load_rows<Q>(wrow, wa);
+            load_rows<Q>(wrow + j2 * Q, wb);
 #pragma unroll
-            for (int a = 0; a < Q; ++a) facc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, facc[a]);
-            j = (j == j1) ? j2 : j + 1;
+            for (int a = 0; a < Q; ++a) facc[a] = lookup_max<Q>(s.tbl_sa, wb[a] + Xb, lookup_max<Q>(s.tbl_sa, wa[a] + Xa, 0u));
+        } else {
+            const int nf = (j1 + 1) + max(D - 1 - j2, 0);
+            int j = 0;
+#pragma unroll 1
+            for (int f = 0; f < nf; ++f) {
+                const uint32_t X32 = expand_x<Q>(xcol[(A + 1 + j) * Q]);
+                uint32_t wr[Q];
+                load_rows<Q>(wrow + j * Q, wr);
+#pragma unroll
+                for (int a = 0; a < Q; ++a) facc[a] = lookup_max<Q>(s.tbl_sa, wr[a] + X32, facc[a]);
+                j = (j == j1) ? j2 : j + 1;
+            }
         }
     }
     // everything the rows below contribute without the wave: bulk and fresh maxima folded once
