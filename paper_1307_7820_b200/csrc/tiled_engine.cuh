@@ -1504,6 +1504,10 @@ static int enqueue_q(rna4r_ctx *ctx, int delta, const uint8_t *seqs, const int64
     // neighbours on its SM (measured at n=6000: 1.98 ms with 2 CTAs/SM, 2.11 ms with 3; n=2000: 0.60 / 0.64); long folds and
     // batches are throughput-bound and take every CTA they can get (n=8000: 3.43 ms with 3, 3.48 with 2; n=16384: 18.8 / 21).
     if (count == 1 && h.max_nt <= 112 && per_sm > 2) per_sm = 2;
+    // Up to n ~ 4000 no super-tile diagonal has more closures in flight than there are SMs, and a closure that has its SM
+    // to itself runs 1.3x faster: one CTA per SM (n = 2000: 0.467 ms against 0.500 with two, n = 4000: 0.969 / 1.031;
+    // n = 5000: 1.469 / 1.361, n = 6000: 2.15 / 1.77 -- there the products need the second CTA)
+    if (count == 1 && h.max_nt <= 64) per_sm = 1;
     if (ctx->max_blocks_per_sm >= 1 && ctx->max_blocks_per_sm < per_sm) per_sm = ctx->max_blocks_per_sm;   // rna4r_set_max_blocks_per_sm
     int blocks = ctx->sm_count * per_sm;
     if ((size_t)blocks > want) blocks = (int)want;
