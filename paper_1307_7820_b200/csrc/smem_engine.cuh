@@ -421,13 +421,18 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
     uint32_t Xp = (uint32_t)vprev;
     int vl = __shfl_sync(FULL, vprev, lane - 1);                  // M(r+1, c-1) for the bottom row
     int v = 0;
+    // the head gather of a row is issued as soon as the row below is known (before the shuffle, the ballot and the
+    // stores of that row): a single warp issues in order, and those would otherwise sit in front of it
+    uint32_t hS = wh[Q - 1] + Xp;
+    uint32_t hR;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(hR) : "r"((hS >> C::ISH) + s.tbl_sa));
 #pragma unroll
     for (int a = Q - 1; a >= 0; --a) {
         // ---- candidates from the rows below: bulk, fresh, pair term (a3), head residual (a5)
         const int lca = __shfl_sync(FULL, Lc, i * Q + a);
         const int vd = (y == 0) ? lca : vl;
         const int cand = max((int)facc[a], vd + (int)((pm >> a) & 1u));
-        const uint32_t best = lookup_max<Q>(s.tbl_sa, wh[a] + Xp, (uint32_t)cand);
+        const uint32_t best = __viaddmax_u16x2(hS, hR, (uint32_t)cand);
         // ---- tail: V(a,y) = max_{y' <= y} C'(a,y') + Qd(y',y)
         uint16_t *row = rowbase + (a & 1) * (C::G * 8);
         if (lane_ok) row[y] = (uint16_t)(best & 0xffffu);
@@ -445,15 +450,19 @@ __device__ __forceinline__ void wave_task(const Params &p, const Sm<Q> &s, int s
             for (int jj = 0; jj < C::NP; ++jj) m2 = __viaddmax_s16x2((int)reinterpret_cast<const uint32_t *>(row)[jj], Qp[jj], m2);
         }
         v = max((int)(short)(m2 & 0xffff), m2 >> 16);
+        // column word: the anchor moves up to row a, the difference to the row below enters at index bit a
+        if (a == Q - 1) Xp = (uint32_t)v;
+        else Xp += (uint32_t)(v - vprev) * (1u + (1u << (C::ISH + a)));
+        if (a > 0) {
+            hS = wh[a - 1] + Xp;
+            asm("ld.shared.u8 %0, [%1];" : "=r"(hR) : "r"((hS >> C::ISH) + s.tbl_sa));
+        }
         // ---- step a6: row word of row r over group B (ballot of the horizontal differences), column word bit
         vl = __shfl_sync(FULL, v, lane - 1);
         RNA4R_CHECK(!own || ((unsigned)(v - vprev) <= 1u && (y == 0 || (unsigned)(v - vl) <= 1u)));   // Lemma 1
         const uint32_t bal = __ballot_sync(FULL, y > 0 && v != vl);
         wout[a] = (((bal >> bsh) & C::HMASK) << 24) | (uint32_t)v;
         rlo[a] = (int16_t)v;
-        // column word: the anchor moves up to row a, the difference to the row below enters at index bit a
-        if (a == Q - 1) Xp = (uint32_t)v;
-        else Xp += (uint32_t)(v - vprev) * (1u + (1u << (C::ISH + a)));
         vprev = v;
         if (own) store_cell<TABLE>(p, s.n, r0 + a, c, v);
     }
