@@ -62,6 +62,7 @@ extern "C" {
 #define RNA4R_ERR_DEVICE     -7   /* no CUDA device, or the device is not compute capability 10.x */
 #define RNA4R_ERR_DTYPE      -8   /* table_dtype not one of RNA4R_TABLE_*                      */
 #define RNA4R_ERR_ENGINE     -9   /* engine id unknown, or the engine does not support this q  */
+#define RNA4R_ERR_SETUP      -10  /* rna4r_fold_static before rna4r_fold_static_setup on this device */
 
 /* ---- per-sequence status bits (device-detected; see rna4r_fold_batch_status) ---- */
 #define RNA4R_STATUS_OK           0
@@ -282,6 +283,37 @@ int rna4r_trace_to_host(rna4r_ctx *ctx, uint64_t *dst_host, int tiles);
  */
 int rna4r_microbench_lookups(rna4r_ctx *ctx, int variant, int iters, int blocks_per_sm, void *workspace_dev,
                              void *stream, float *ms_host, double *lookups_host);
+
+/*
+ * A fold that allocates nothing and takes no workspace, for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it).  The same fill as rna4r_fold with
+ * RNA4R_ENGINE_TILED, score only (D(1,n) of eq. (1)), whatever engine the context is set to; its
+ * scratch (plan, flags, super-tile records, bulk maxima) is a static device array inside the library of
+ * RNA4R_STATIC_SCRATCH_BYTES, which every GPU that loads the library holds until the process exits.
+ *
+ *   rna4r_fold_static_setup   once per device (any context of that device, q <= 11; repeat it for every q used, it
+ *                             also warms that q's kernels up): looks the array's device address up, runs one
+ *                             100-base fold out of the array's tail on `stream` and synchronises that stream.  Not
+ *                             for use under graph capture.  Errors: CONTEXT, ENGINE (q = 12), DEVICE, CUDA.
+ *   rna4r_fold_static_max_n   largest n whose scratch fits the array for the context's q (1567 at q = 2, 1951 at q = 4,
+ *                             2239 at q = 8, 2375 at q = 11), or a
+ *                             negative error code (CONTEXT, ENGINE).
+ *   rna4r_fold_static         seq_dev: DEVICE, n ASCII bases (not modified; may be NULL if n == 0); score_out_dev:
+ *                             DEVICE int32, written when the stream work completes (-1 for a byte that is not a base,
+ *                             reading g4).  Enqueues on `stream` and returns; calls no cudaMalloc / cudaFree or
+ *                             allocating routine.  Errors: CONTEXT, ENGINE (q = 12), NULL, BAD_N (n < 0 or
+ *                             n > rna4r_fold_static_max_n: nothing is enqueued), SETUP (rna4r_fold_static_setup has
+ *                             not run on this device in this process), CUDA.
+ *
+ * Every call on a device shares the one array, whatever its context or stream, and the array keeps the last
+ * call's contents: each fold zeroes the part that has to start at zero itself, but two calls whose GPU work
+ * overlaps (different streams without an ordering between them, or two host threads) race.  Order them on one
+ * stream or with events.  The process-wide setup state is not guarded against concurrent setup calls.
+ */
+#define RNA4R_STATIC_SCRATCH_BYTES (8u << 20)
+int rna4r_fold_static_setup(rna4r_ctx *ctx, void *stream);
+int rna4r_fold_static_max_n(const rna4r_ctx *ctx);
+int rna4r_fold_static(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_out_dev, void *stream);
 
 /* cudaError_t of the most recent failing CUDA call on this context (0 if none). */
 int rna4r_last_cuda_error(const rna4r_ctx *ctx);

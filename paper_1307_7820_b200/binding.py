@@ -74,6 +74,9 @@ def load():
     L.rna4r_trace_to_host.argtypes = [vp, vp, ctypes.c_int]
     L.rna4r_last_launch_count.argtypes = [vp]
     L.rna4r_last_cuda_error.argtypes = [vp]
+    L.rna4r_fold_static_setup.argtypes = [vp, vp]
+    L.rna4r_fold_static_max_n.argtypes = [vp]
+    L.rna4r_fold_static.argtypes = [vp, vp, ctypes.c_int, vp, vp]
     _lib = L
     return L
 
@@ -221,6 +224,23 @@ class Rna4r:
                                    table_out.data_ptr() if table_out is not None else None, table_dtype,
                                    workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)), "rna4r_fold")
         return score_out, table_out
+
+    def fold_static_setup(self, stream=None):
+        """rna4r_fold_static_setup: once per device (and per q), before fold_static."""
+        _check(self.lib.rna4r_fold_static_setup(self.h, _stream_ptr(stream)), "rna4r_fold_static_setup")
+
+    def fold_static_max_n(self) -> int:
+        n = self.lib.rna4r_fold_static_max_n(self.h)
+        _check(min(n, 0), "rna4r_fold_static_max_n")
+        return n
+
+    def fold_static(self, seq_dev, score_out, n: int | None = None, stream=None):
+        """rna4r_fold_static: score-only fold out of the library's static scratch array; allocates nothing (the caller
+        passes the int32[1] CUDA tensor score_out).  Enqueues only."""
+        n = int(seq_dev.numel()) if n is None else n
+        _check(self.lib.rna4r_fold_static(self.h, seq_dev.data_ptr() if n else None, n, score_out.data_ptr(),
+                                          _stream_ptr(stream)), "rna4r_fold_static")
+        return score_out
 
     def fold_batch(self, seqs_dev, offsets_dev, lens_host: np.ndarray, scores_out=None, workspace=None, stream=None,
                    status_out=None):

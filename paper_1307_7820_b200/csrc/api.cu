@@ -128,6 +128,7 @@ const char *rna4r_strerror(int code)
     case RNA4R_ERR_DEVICE: return "no sm_100 CUDA device (there is no CPU fallback)";
     case RNA4R_ERR_DTYPE: return "bad table dtype";
     case RNA4R_ERR_ENGINE: return "unknown engine, or engine does not support this q";
+    case RNA4R_ERR_SETUP: return "rna4r_fold_static before rna4r_fold_static_setup on this device";
     default: return "unknown error code";
     }
 }
@@ -605,6 +606,78 @@ int rna4r_fold_batch_host(rna4r_ctx *ctx, const uint8_t *seqs_host, const int32_
     RNA4R_CUDA(ctx, cudaStreamSynchronize(st));
     ctx->last_launches = launches;
     return RNA4R_OK;
+}
+
+
+// ---- rna4r_fold_static: a fold that allocates nothing and takes no workspace (include/rna4r.h) ------------------------
+// The scratch of the tiled engine (plan, flags, super-tile records, bulk maxima) lives in this file-scope device array:
+// RNA4R_STATIC_SCRATCH_BYTES on every GPU that loads the library, until the process exits.  In host code the NAME of the
+// array is a host-side stand-in, not a device address: the address the kernels get is asked for once per device with
+// cudaGetSymbolAddress (rna4r_fold_static_setup) and kept in g_static_scratch[device].
+static __device__ __align__(256) unsigned char rna4r_static_scratch[RNA4R_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t kStaticTail = 512;                  // end of the array: the warm-up fold's sequence (256 B) and score
+void *g_static_scratch[kStaticMaxDevices] = {nullptr};
+
+inline size_t static_ws_limit() { return (size_t)RNA4R_STATIC_SCRATCH_BYTES - kStaticTail; }
+
+int static_enqueue(rna4r_ctx *ctx, void *scratch, const uint8_t *seq_dev, int n, int32_t *score_dev, cudaStream_t st)
+{
+    // the tiled engine zeroes the prefix of its workspace that has to start at zero (plan header, flags) in every fold
+    return dispatch_q(ctx->q, [&](auto Q) {
+        return tiled::enqueue_q<decltype(Q)::value>(ctx, kDelta, seq_dev, nullptr, nullptr, 1, n, score_dev, nullptr, nullptr,
+                                                    RNA4R_TABLE_NONE, scratch, st);
+    });
+}
+}  // namespace
+
+int rna4r_fold_static_max_n(const rna4r_ctx *ctx)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (ctx->q > 11) return RNA4R_ERR_ENGINE;
+    int lo = 0, hi = 65534;                          // the workspace grows with n
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) / 2;
+        if (tiled_ws(ctx, nullptr, 1, mid) <= static_ws_limit()) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+int rna4r_fold_static_setup(rna4r_ctx *ctx, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (ctx->q > 11) return RNA4R_ERR_ENGINE;
+    if (ctx->device < 0 || ctx->device >= kStaticMaxDevices) return RNA4R_ERR_DEVICE;
+    cudaStream_t st = (cudaStream_t)stream;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    void *ptr = nullptr;
+    RNA4R_CUDA(ctx, cudaGetSymbolAddress(&ptr, rna4r_static_scratch));
+    if (!ptr) return RNA4R_ERR_CUDA;
+    // warm-up fold of 100 x 'A' out of the array's tail: module loading, kernel attributes and the occupancy query of
+    // this context's q happen here, not in the first rna4r_fold_static call
+    unsigned char *tailp = (unsigned char *)ptr + static_ws_limit();
+    RNA4R_CUDA(ctx, cudaMemsetAsync(tailp, 'A', 256, st));
+    int rc = static_enqueue(ctx, ptr, tailp, 100, (int32_t *)(tailp + 256), st);
+    if (rc != RNA4R_OK) return rc;
+    RNA4R_CUDA(ctx, cudaStreamSynchronize(st));
+    g_static_scratch[ctx->device] = ptr;
+    return RNA4R_OK;
+}
+
+int rna4r_fold_static(rna4r_ctx *ctx, const uint8_t *seq_dev, int n, int32_t *score_out_dev, void *stream)
+{
+    if (!ctx_ok(ctx)) return RNA4R_ERR_CONTEXT;
+    if (ctx->q > 11) return RNA4R_ERR_ENGINE;
+    if (!score_out_dev || (!seq_dev && n > 0)) return RNA4R_ERR_NULL;
+    if (n < 0 || n > 65534) return RNA4R_ERR_BAD_N;
+    if (tiled_ws(ctx, nullptr, 1, n) > static_ws_limit()) return RNA4R_ERR_BAD_N;       // beyond rna4r_fold_static_max_n
+    if (ctx->device < 0 || ctx->device >= kStaticMaxDevices) return RNA4R_ERR_DEVICE;
+    void *scratch = g_static_scratch[ctx->device];
+    if (!scratch) return RNA4R_ERR_SETUP;
+    RNA4R_CUDA(ctx, cudaSetDevice(ctx->device));
+    return static_enqueue(ctx, scratch, seq_dev, n, score_out_dev, (cudaStream_t)stream);
 }
 
 }  // extern "C"

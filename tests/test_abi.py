@@ -58,7 +58,7 @@ def test_strerror_and_version_need_no_gpu():
     L = load()
     assert L.rna4r_version().decode().startswith("rna4r")
     assert L.rna4r_strerror(0).decode() == "ok"
-    for code in range(-9, 0):
+    for code in range(-10, 0):
         assert len(L.rna4r_strerror(code).decode()) > 3
 
 
